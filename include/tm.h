@@ -1,0 +1,171 @@
+/*
+ * tm.h -- C ABI of the B200-native twisted-mass dslash / MdagM / CG / loop library (libtm_b200.so).
+ *
+ * Hot path of arxiv/paper_1309_2256 ("Evaluation of disconnected quark loops for hadron structure using GPUs").
+ * Citations are PAPER.md:<line> plus section / equation.  Readings of the paper are listed in DESIGN.md.
+ *
+ * General rules
+ *  - Plain C types only.  `stream` arguments are a cudaStream_t passed as void* (NULL = legacy default stream).
+ *  - OWNERSHIP: the caller owns all device memory.  The library never allocates device memory; workspaces are
+ *    passed in, sized by the tm_*_bytes() queries.  Pointers are borrowed until the stream work completes.
+ *    Every device buffer must be 256-byte aligned.  "device" / "host" is stated per argument.
+ *  - ERRORS: every entry point returns int: TM_OK (0) or a negative tm_status.  No exceptions, no exit().
+ *    Calls are asynchronous on `stream` unless they fill host structs (tm_cg*, tm_tsm_batch_host: documented).
+ *  - There is no CPU fallback: without a CUDA device every compute call returns TM_ERR_CUDA.
+ *
+ * Conventions (identical to the oracle's, DESIGN.md section "Readings")
+ *  - Lattice X x Y x Z x T, all even and >= 4; site = x + X*(y + Y*(z + Z*t)); mu = 0..3 = x,y,z,t;
+ *    parity = (x+y+z+t)&1, even = 0.  Periodic in space, time antiperiodic if the lattice was created so.
+ *  - Canonical fields (fp64, complex interleaved): gauge U[site][mu][row][col][re,im],
+ *    spinor psi[site][spin][colour][re,im].
+ *  - Dslash = positive hopping sum
+ *      (Dslash psi)(x) = sum_mu (1-g_mu) s_mu(x) U_mu(x) psi(x+mu) + (1+g_mu) s_mu(x-mu) U_mu(x-mu)^dag psi(x-mu),
+ *    M(kappa,mu) = 1 + i a g5 - kappa Dslash, a = 2 kappa mu  (PAPER.md:162 Eq. 16 B, H; :367 Eq. A1).
+ *    Chiral gamma basis: g_k = [[0,-i s_k],[i s_k,0]], g_4 = [[0,1],[1,0]], g5 = diag(1,1,-1,-1).
+ *  - Packed device layout: per parity, checkerboard index cb = site>>1;
+ *    structure of arrays in 16-byte chunks [chunk][cb]; fp16 spinors carry one fp32 norm per site.
+ */
+#ifndef TM_B200_H
+#define TM_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TM_VERSION 100
+
+typedef struct tm_lattice tm_lattice; /* opaque host-side geometry descriptor */
+
+typedef enum { TM_PREC_F64 = 8, TM_PREC_F32 = 4, TM_PREC_F16 = 2 } tm_prec;   /* storage bytes per real */
+typedef enum { TM_RECON_18 = 18, TM_RECON_12 = 12 } tm_recon;                /* reals stored per link */
+typedef enum { TM_KIND_PLAIN = 0, TM_KIND_TWIST_INV = 1, TM_KIND_XPAY_TWIST = 2 } tm_dslash_kind;
+typedef enum { TM_CG_HP_MIXED = 0, TM_CG_LP_TRUNCATED = 1 } tm_cg_mode;
+
+typedef enum {
+    TM_OK = 0,
+    TM_ERR_ARG = -1,       /* null pointer, bad enum, aliasing out == in, nrhs out of range */
+    TM_ERR_LAYOUT = -2,    /* dims odd or < 4, misaligned buffer, workspace too small */
+    TM_ERR_NOT_SU3 = -3,   /* tm_gauge_pack with recon 12: a link is farther than su3_tol from SU(3) */
+    TM_ERR_CUDA = -4,      /* CUDA runtime error (no device, launch failure); tm_last_cuda_error() has the text */
+    TM_ERR_BREAKDOWN = -5, /* CG: <p,Ap> <= 0 or NaN */
+    TM_ERR_MAXITER = -6    /* CG: max_iter reached before tol (solution still returned) */
+} tm_status;
+
+#define TM_MAX_NRHS 16
+
+int tm_version(void);
+const char* tm_strerror(int status);
+const char* tm_last_cuda_error(void);
+
+/* ---- geometry ------------------------------------------------------------------------------------------ */
+/* dims = {X,Y,Z,T}.  antiperiodic_t != 0: hops across t = T-1 <-> 0 carry -1 (BASELINE.json configs[0]). */
+int tm_lattice_create(tm_lattice** L, const int dims[4], int antiperiodic_t);
+void tm_lattice_destroy(tm_lattice* L);
+
+/* ---- sizes --------------------------------------------------------------------------------------------- */
+size_t tm_gauge_bytes(const tm_lattice* L, int prec, int recon);
+/* full != 0: both parities ([even block][odd block]); else one parity.  nrhs fields are stacked [rhs][...]. */
+size_t tm_spinor_bytes(const tm_lattice* L, int prec, int full, int nrhs);
+
+/* ---- a0: gauge pack (links stored with 12 parameters and rebuilt on the fly) ------------- */
+/* U_canonical: DEVICE, fp64 canonical, 4*V*18 doubles.  packed_out: DEVICE, tm_gauge_bytes().
+ * recon 12 keeps rows 0,1 (row 2 = conj(row0 x row1) is rebuilt in the kernels; the antiperiodic sign is NOT
+ * folded into stored links).  With recon 12, returns TM_ERR_NOT_SU3 if max |U U^dag - 1|, |row2 - conj(r0 x r1)|
+ * exceeds su3_tol (this check synchronises the stream); su3_tol <= 0 skips the check. */
+int tm_gauge_pack(const tm_lattice* L, const double* U_canonical, int prec, int recon, void* packed_out,
+                  double su3_tol, void* stream);
+
+/* ---- a1: spinor pack / unpack (both parities, nrhs fields) ----------------------------------------------- */
+/* psi_canonical: DEVICE fp64 [nrhs][V][4][3][2]; packed: DEVICE [nrhs][parity][...] at `prec`.
+ * fp16: per-site fp32 norm = max |re|,|im| over the site's 24 reals, components stored as x/norm (RN). */
+int tm_spinor_pack(const tm_lattice* L, const double* psi_canonical, int prec, int nrhs, void* packed_out, void* stream);
+int tm_spinor_unpack(const tm_lattice* L, const void* packed, int prec, int nrhs, double* psi_canonical, void* stream);
+/* Z2 x iZ2 noise from 2-bit codes: codes DEVICE uint8 [nrhs][V][12], bit0 = re<0, bit1 = im<0;
+ * value = (+-1 +- i)/sqrt(2). */
+int tm_spinor_pack_z4(const tm_lattice* L, const unsigned char* codes, int prec, int nrhs, void* packed_out, void* stream);
+
+/* ---- a2+a3: hopping term with fused local epilogue ("fused CUDA kernels, such as R_oo^-1 Dslash_oe,
+ *      (R_ee - kappa^2 Dslash_eo) (and their daggered analogues)") ----------------------------------------- */
+/* out (parity out_parity) = epilogue(Dslash_{out_parity <- other} in).  in/out/x: DEVICE one-parity packed spinors
+ * ([rhs][...] stacked, nrhs <= TM_MAX_NRHS), gauge: DEVICE packed links.  out must not alias in.
+ *   PLAIN:       out = D in                    (D = Dslash, or Dslash^dag if dagger)
+ *   TWIST_INV:   out = R(+-a)^-1 D in          (a = 2 kappa mu; sign - if dagger)
+ *   XPAY_TWIST:  out = R(+-a) x - kappa^2 D in (x: same parity as out)
+ * flops per output site counted as 1320 / 1392 / 1416. */
+int tm_dslash(const tm_lattice* L, const void* gauge, int prec, int recon, void* out, const void* in, const void* x_or_null,
+              int out_parity, int dagger, int kind, double kappa, double mu, int nrhs, void* stream);
+/* general epilogue: out = (p0 + i p1 g5) x + (q0 + i q1 g5) (D in), pq = {p0,p1,q0,q1}; x may be NULL iff p0=p1=0. */
+int tm_dslash_general(const tm_lattice* L, const void* gauge, int prec, int recon, void* out, const void* in,
+                      const void* x_or_null, int out_parity, int dagger, const double pq[4], int nrhs, void* stream);
+
+/* ---- a4: normal operator of the asymmetric even-odd system (PAPER.md:373 Eq. A2 lhs) ---------------------- */
+/* out = M_pc^dag M_pc in on `parity`, M_pc = R - kappa^2 Dslash R^-1 Dslash; tmp: DEVICE, 2 one-parity spinors of nrhs. */
+int tm_MdagM(const tm_lattice* L, const void* gauge, int prec, int recon, void* out, const void* in, void* tmp, int parity,
+             double kappa, double mu, int nrhs, void* stream);
+
+/* ---- a5-a7: CG ("the inverter, which is a Conjugate Gradient (CG) solver in this work, is truncated ...
+ *      |r| < 10^-2 ... or a fixed number of iterations") --------------------------------------------------- */
+typedef struct {
+    double kappa, mu;
+    double tol;            /* stop when |r_k| <= tol |b''| (iterated residual of the normal system); 0: run max_iter */
+    int max_iter;
+    int mode;              /* tm_cg_mode */
+    double reliable_delta; /* HP_MIXED: recompute the true residual in prec_hp when |r| drops by this factor (0 -> 0.1) */
+    int check_every;       /* host polls the device convergence flag every this many iterations (0 -> 4) */
+} tm_cg_params;
+
+typedef struct {
+    int iters;             /* CG iterations performed (all in prec_lp for HP_MIXED) */
+    int status;            /* tm_status of this solve */
+    int reliable_updates;  /* HP_MIXED only */
+    double iterated_resid; /* |r_k| / |b''| */
+    double true_resid;     /* |b'' - A x| / |b''| recomputed in the HP precision (LP mode: in prec_lp arithmetic) */
+} tm_cg_info;
+
+/* Solve M(kappa,mu) s = eta on the full lattice through the even-even Schur system, x0 = 0:
+ *   b' = eta_e + kappa Dslash_eo R^-1 eta_o; b'' = M_pc^dag b'; CG on M_pc^dag M_pc; s_o = R^-1 (eta_o + kappa Dslash_oe s_e).
+ * HP_MIXED: eta/s packed full-lattice at prec_hp; iterations in prec_lp with reliable updates in prec_hp.
+ * LP_TRUNCATED: eta/s packed at prec_lp, everything in prec_lp storage (fp32 arithmetic, fp64 reductions), no correction;
+ *   gauge_hp may be NULL.
+ * info: HOST.  The call synchronises `stream` before returning.  nrhs right-hand sides share every gauge load;
+ * each has its own alpha, beta and stops updating at its own convergence (info[nrhs]). */
+size_t tm_cg_workspace_bytes(const tm_lattice* L, int prec_hp, int prec_lp, int mode, int nrhs);
+int tm_cg_multi(const tm_lattice* L, const void* gauge_hp, int prec_hp, const void* gauge_lp, int prec_lp, int recon,
+                void* s_full, const void* eta_full, const tm_cg_params* p, int nrhs, tm_cg_info* info, void* workspace,
+                size_t workspace_bytes, void* stream);
+/* tm_cg == tm_cg_multi with nrhs = 1 */
+int tm_cg(const tm_lattice* L, const void* gauge_hp, int prec_hp, const void* gauge_lp, int prec_lp, int recon, void* s_full,
+          const void* eta_full, const tm_cg_params* p, tm_cg_info* info, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- a8: loop contraction (PAPER.md:116 Eq. 10; :411 colour trace, Dirac indices open) --------------------- */
+/* out[rhs][n][t] = sum_{x: x4=t} a(x)^dag (Gamma_n x 1) b(x), Gamma_n = g1^b0 g2^b1 g3^b2 g4^b3, n = b0+2b1+4b2+8b3.
+ * a_full, b_full: DEVICE packed full-lattice spinors [nrhs][parity][...]; out: DEVICE double [nrhs][16][T][2].
+ * Fixed-order two-stage reduction (bit-reproducible). */
+size_t tm_loop_workspace_bytes(const tm_lattice* L, int nrhs);
+int tm_loop_contract(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, double* out,
+                     void* workspace, void* stream);
+
+/* ---- end-to-end TSM batch with HOST buffers ("the source is sent to the GPUs for inversion and
+ *      contraction, and contractions are stored back in the CPUs") ----------------------------------------- */
+/* codes_host: HOST (pinned recommended) uint8 [nrhs][V][12] Z2xiZ2 codes; loops_host: HOST double [nrhs][16][T][2].
+ * Copies the codes H2D, packs, runs tm_cg_multi (LP_TRUNCATED), contracts eta^dag Gamma_n s, copies the loops D2H,
+ * synchronises.  workspace: DEVICE, tm_tsm_workspace_bytes(). */
+size_t tm_tsm_workspace_bytes(const tm_lattice* L, int prec_lp, int nrhs);
+int tm_tsm_batch_host(const tm_lattice* L, const void* gauge_lp, int prec_lp, int recon, const unsigned char* codes_host,
+                      const tm_cg_params* p, int nrhs, tm_cg_info* info, double* loops_host, void* workspace,
+                      size_t workspace_bytes, void* stream);
+
+/* ---- instrumentation ------------------------------------------------------------------------------------- */
+/* Number of kernels this library has launched since load (all entry points). */
+unsigned long long tm_launch_count(void);
+/* When enabled, every dslash-family launch is bracketed by CUDA events on its stream; tm_kernel_timing_read
+ * synchronises and returns the accumulated milliseconds and launch count since the last reset. */
+int tm_kernel_timing_enable(int on);
+int tm_kernel_timing_read(double* ms_total, long long* launches, int reset);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

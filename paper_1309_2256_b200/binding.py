@@ -1,0 +1,267 @@
+"""ctypes binding of include/tm.h.  Function names and argument order follow the header one to one."""
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtm_b200.so")
+
+TM_PREC_F64, TM_PREC_F32, TM_PREC_F16 = 8, 4, 2
+TM_RECON_18, TM_RECON_12 = 18, 12
+TM_KIND_PLAIN, TM_KIND_TWIST_INV, TM_KIND_XPAY_TWIST = 0, 1, 2
+TM_CG_HP_MIXED, TM_CG_LP_TRUNCATED = 0, 1
+TM_OK, TM_ERR_ARG, TM_ERR_LAYOUT, TM_ERR_NOT_SU3, TM_ERR_CUDA, TM_ERR_BREAKDOWN, TM_ERR_MAXITER = 0, -1, -2, -3, -4, -5, -6
+TM_MAX_NRHS = 16
+
+ABI_SYMBOLS = [
+    "tm_version", "tm_strerror", "tm_last_cuda_error", "tm_lattice_create", "tm_lattice_destroy", "tm_gauge_bytes",
+    "tm_spinor_bytes", "tm_gauge_pack", "tm_spinor_pack", "tm_spinor_unpack", "tm_spinor_pack_z4", "tm_dslash",
+    "tm_dslash_general", "tm_MdagM", "tm_cg_workspace_bytes", "tm_cg_multi", "tm_cg", "tm_loop_workspace_bytes",
+    "tm_loop_contract", "tm_tsm_workspace_bytes", "tm_tsm_batch_host", "tm_launch_count", "tm_kernel_timing_enable",
+    "tm_kernel_timing_read",
+]
+
+
+class tm_cg_params(ctypes.Structure):
+    _fields_ = [("kappa", ctypes.c_double), ("mu", ctypes.c_double), ("tol", ctypes.c_double), ("max_iter", ctypes.c_int),
+                ("mode", ctypes.c_int), ("reliable_delta", ctypes.c_double), ("check_every", ctypes.c_int)]
+
+
+class tm_cg_info(ctypes.Structure):
+    _fields_ = [("iters", ctypes.c_int), ("status", ctypes.c_int), ("reliable_updates", ctypes.c_int),
+                ("iterated_resid", ctypes.c_double), ("true_resid", ctypes.c_double)]
+
+
+class TmError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        msg = "%s: %s" % (where, tm_strerror(status))
+        if status == TM_ERR_CUDA:
+            msg += " [" + tm_last_cuda_error() + "]"
+        super().__init__(msg)
+
+
+_lib = None
+
+
+def load():
+    """Load libtm_b200.so; fails loudly if it has not been built (python -m paper_1309_2256_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libtm_b200.so is missing: run `python -m paper_1309_2256_b200.build` (there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i, d, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+    P = ctypes.POINTER
+    sig = {
+        "tm_version": (i, []),
+        "tm_strerror": (ctypes.c_char_p, [i]),
+        "tm_last_cuda_error": (ctypes.c_char_p, []),
+        "tm_lattice_create": (i, [P(vp), P(i), i]),
+        "tm_lattice_destroy": (None, [vp]),
+        "tm_gauge_bytes": (sz, [vp, i, i]),
+        "tm_spinor_bytes": (sz, [vp, i, i, i]),
+        "tm_gauge_pack": (i, [vp, vp, i, i, vp, d, vp]),
+        "tm_spinor_pack": (i, [vp, vp, i, i, vp, vp]),
+        "tm_spinor_unpack": (i, [vp, vp, i, i, vp, vp]),
+        "tm_spinor_pack_z4": (i, [vp, vp, i, i, vp, vp]),
+        "tm_dslash": (i, [vp, vp, i, i, vp, vp, vp, i, i, i, d, d, i, vp]),
+        "tm_dslash_general": (i, [vp, vp, i, i, vp, vp, vp, i, i, P(d), i, vp]),
+        "tm_MdagM": (i, [vp, vp, i, i, vp, vp, vp, i, d, d, i, vp]),
+        "tm_cg_workspace_bytes": (sz, [vp, i, i, i, i]),
+        "tm_cg_multi": (i, [vp, vp, i, vp, i, i, vp, vp, P(tm_cg_params), i, P(tm_cg_info), vp, sz, vp]),
+        "tm_cg": (i, [vp, vp, i, vp, i, i, vp, vp, P(tm_cg_params), P(tm_cg_info), vp, sz, vp]),
+        "tm_loop_workspace_bytes": (sz, [vp, i]),
+        "tm_loop_contract": (i, [vp, vp, vp, i, i, vp, vp, vp]),
+        "tm_tsm_workspace_bytes": (sz, [vp, i, i]),
+        "tm_tsm_batch_host": (i, [vp, vp, i, i, vp, P(tm_cg_params), i, P(tm_cg_info), vp, vp, sz, vp]),
+        "tm_launch_count": (ctypes.c_ulonglong, []),
+        "tm_kernel_timing_enable": (i, [i]),
+        "tm_kernel_timing_read": (i, [P(d), P(ctypes.c_longlong), i]),
+    }
+    for name, (res, args) in sig.items():
+        f = getattr(lib, name)
+        f.restype = res
+        f.argtypes = args
+    _lib = lib
+    return lib
+
+
+def _ptr(t):
+    """Device/host pointer of a torch tensor or numpy array (None -> NULL)."""
+    if t is None:
+        return None
+    if isinstance(t, torch.Tensor):
+        return ctypes.c_void_p(t.data_ptr())
+    if isinstance(t, np.ndarray):
+        return ctypes.c_void_p(t.ctypes.data)
+    return ctypes.c_void_p(int(t))
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def _check(rc, where, allow=()):
+    if rc != TM_OK and rc not in allow:
+        raise TmError(rc, where)
+    return rc
+
+
+def tm_version():
+    return load().tm_version()
+
+
+def tm_strerror(status):
+    return load().tm_strerror(status).decode()
+
+
+def tm_last_cuda_error():
+    return load().tm_last_cuda_error().decode()
+
+
+class Lattice:
+    """Owns a tm_lattice* (host-side geometry descriptor)."""
+
+    def __init__(self, dims, antiperiodic_t=True):
+        self.dims = tuple(int(d) for d in dims)
+        self.antiperiodic_t = bool(antiperiodic_t)
+        h = ctypes.c_void_p()
+        arr = (ctypes.c_int * 4)(*self.dims)
+        _check(load().tm_lattice_create(ctypes.byref(h), arr, int(antiperiodic_t)), "tm_lattice_create")
+        self.handle = h
+        X, Y, Z, T = self.dims
+        self.V = X * Y * Z * T
+        self.T = T
+
+    def __del__(self):
+        try:
+            if getattr(self, "handle", None):
+                load().tm_lattice_destroy(self.handle)
+                self.handle = None
+        except Exception:
+            pass
+
+
+def tm_lattice_create(dims, antiperiodic_t=True):
+    return Lattice(dims, antiperiodic_t)
+
+
+def tm_gauge_bytes(L, prec, recon):
+    return load().tm_gauge_bytes(L.handle, prec, recon)
+
+
+def tm_spinor_bytes(L, prec, full, nrhs=1):
+    return load().tm_spinor_bytes(L.handle, prec, int(full), nrhs)
+
+
+def tm_gauge_pack(L, U_canonical, prec, recon, packed_out, su3_tol=1e-10, stream=None):
+    return _check(load().tm_gauge_pack(L.handle, _ptr(U_canonical), prec, recon, _ptr(packed_out), su3_tol, _stream(stream)),
+                  "tm_gauge_pack")
+
+
+def tm_spinor_pack(L, psi_canonical, prec, nrhs, packed_out, stream=None):
+    return _check(load().tm_spinor_pack(L.handle, _ptr(psi_canonical), prec, nrhs, _ptr(packed_out), _stream(stream)), "tm_spinor_pack")
+
+
+def tm_spinor_unpack(L, packed, prec, nrhs, psi_canonical, stream=None):
+    return _check(load().tm_spinor_unpack(L.handle, _ptr(packed), prec, nrhs, _ptr(psi_canonical), _stream(stream)), "tm_spinor_unpack")
+
+
+def tm_spinor_pack_z4(L, codes, prec, nrhs, packed_out, stream=None):
+    return _check(load().tm_spinor_pack_z4(L.handle, _ptr(codes), prec, nrhs, _ptr(packed_out), _stream(stream)), "tm_spinor_pack_z4")
+
+
+def tm_dslash(L, gauge, prec, recon, out, inp, x, out_parity, dagger, kind, kappa, mu, nrhs=1, stream=None):
+    return _check(load().tm_dslash(L.handle, _ptr(gauge), prec, recon, _ptr(out), _ptr(inp), _ptr(x), out_parity, int(dagger), kind,
+                                   kappa, mu, nrhs, _stream(stream)), "tm_dslash")
+
+
+def tm_dslash_general(L, gauge, prec, recon, out, inp, x, out_parity, dagger, pq, nrhs=1, stream=None):
+    arr = (ctypes.c_double * 4)(*pq)
+    return _check(load().tm_dslash_general(L.handle, _ptr(gauge), prec, recon, _ptr(out), _ptr(inp), _ptr(x), out_parity, int(dagger),
+                                           arr, nrhs, _stream(stream)), "tm_dslash_general")
+
+
+def tm_MdagM(L, gauge, prec, recon, out, inp, tmp, parity, kappa, mu, nrhs=1, stream=None):
+    return _check(load().tm_MdagM(L.handle, _ptr(gauge), prec, recon, _ptr(out), _ptr(inp), _ptr(tmp), parity, kappa, mu, nrhs,
+                                  _stream(stream)), "tm_MdagM")
+
+
+def tm_cg_workspace_bytes(L, prec_hp, prec_lp, mode, nrhs=1):
+    return load().tm_cg_workspace_bytes(L.handle, prec_hp, prec_lp, mode, nrhs)
+
+
+def make_cg_params(kappa, mu, tol, max_iter, mode, reliable_delta=0.1, check_every=4):
+    return tm_cg_params(kappa, mu, tol, max_iter, mode, reliable_delta, check_every)
+
+
+_SOFT = (TM_ERR_MAXITER, TM_ERR_BREAKDOWN)
+
+
+def tm_cg_multi(L, gauge_hp, prec_hp, gauge_lp, prec_lp, recon, s_full, eta_full, params, nrhs, workspace, stream=None):
+    """Returns (status, [tm_cg_info]*nrhs); MAXITER / BREAKDOWN are returned, not raised."""
+    info = (tm_cg_info * nrhs)()
+    ws_bytes = workspace.numel() * workspace.element_size()
+    rc = load().tm_cg_multi(L.handle, _ptr(gauge_hp), prec_hp, _ptr(gauge_lp), prec_lp, recon, _ptr(s_full), _ptr(eta_full),
+                            ctypes.byref(params), nrhs, info, _ptr(workspace), ws_bytes, _stream(stream))
+    _check(rc, "tm_cg_multi", allow=_SOFT)
+    return rc, list(info)
+
+
+def tm_cg(L, gauge_hp, prec_hp, gauge_lp, prec_lp, recon, s_full, eta_full, params, workspace, stream=None):
+    rc, info = tm_cg_multi(L, gauge_hp, prec_hp, gauge_lp, prec_lp, recon, s_full, eta_full, params, 1, workspace, stream)
+    return rc, info[0]
+
+
+def tm_loop_workspace_bytes(L, nrhs=1):
+    return load().tm_loop_workspace_bytes(L.handle, nrhs)
+
+
+def tm_loop_contract(L, a_full, b_full, prec, nrhs, out, workspace, stream=None):
+    return _check(load().tm_loop_contract(L.handle, _ptr(a_full), _ptr(b_full), prec, nrhs, _ptr(out), _ptr(workspace), _stream(stream)),
+                  "tm_loop_contract")
+
+
+def tm_tsm_workspace_bytes(L, prec_lp, nrhs):
+    return load().tm_tsm_workspace_bytes(L.handle, prec_lp, nrhs)
+
+
+def tm_tsm_batch_host(L, gauge_lp, prec_lp, recon, codes_host, params, nrhs, loops_host, workspace, stream=None):
+    info = (tm_cg_info * nrhs)()
+    ws_bytes = workspace.numel() * workspace.element_size()
+    rc = load().tm_tsm_batch_host(L.handle, _ptr(gauge_lp), prec_lp, recon, _ptr(codes_host), ctypes.byref(params), nrhs, info,
+                                  _ptr(loops_host), _ptr(workspace), ws_bytes, _stream(stream))
+    _check(rc, "tm_tsm_batch_host", allow=_SOFT)
+    return rc, list(info)
+
+
+def tm_launch_count():
+    return int(load().tm_launch_count())
+
+
+def tm_kernel_timing_enable(on):
+    return _check(load().tm_kernel_timing_enable(int(on)), "tm_kernel_timing_enable")
+
+
+def tm_kernel_timing_read(reset=True):
+    ms = ctypes.c_double()
+    n = ctypes.c_longlong()
+    _check(load().tm_kernel_timing_read(ctypes.byref(ms), ctypes.byref(n), int(reset)), "tm_kernel_timing_read")
+    return ms.value, n.value
+
+
+def device_buffer(nbytes, device="cuda"):
+    """Plumbing: a 256-byte aligned uint8 device buffer owned by PyTorch."""
+    t = torch.empty(int(nbytes) + 256, dtype=torch.uint8, device=device)
+    off = (-t.data_ptr()) % 256
+    return t[off:off + int(nbytes)]
+
+
+__all__ = [n for n in dir() if n.startswith(("tm_", "TM_"))] + ["Lattice", "TmError", "make_cg_params", "device_buffer", "load",
+                                                                 "LIB_PATH", "ABI_SYMBOLS"]

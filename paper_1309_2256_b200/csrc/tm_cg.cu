@@ -1,0 +1,446 @@
+// tm_cg.cu -- a6 / a7 of SURVEY.md 8(a): CG on the even-even Schur system, truncated LP mode batched over
+// right-hand sides, mixed-precision HP mode with reliable updates, and the host-buffer TSM batch entry point.
+//
+//   b' = eta_e + kappa Dslash_eo R^-1 eta_o;  b'' = M_pc^dag b';  CG on A = M_pc^dag M_pc, x0 = 0;
+//   s_e = x;  s_o = R^-1 (eta_o + kappa Dslash_oe s_e)                 (PAPER.md:373-381 Eq. A2, A4 as corrected
+//   in DESIGN.md reading 6; PAPER.md:67 for the truncation rule)
+#include "tm_blas.cuh"
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+namespace tmk {
+
+template <typename F>
+static inline int by_prec(int prec, F&& f)
+{
+    if (prec == 8) return f(std::integral_constant<int, 8>());
+    if (prec == 4) return f(std::integral_constant<int, 4>());
+    return f(std::integral_constant<int, 2>());
+}
+
+static inline VecArg V_(void* p, size_t stride) { return VecArg{static_cast<char*>(p), stride}; }
+static inline VecArg V_(const void* p, size_t stride) { return VecArg{static_cast<char*>(const_cast<void*>(p)), stride}; }
+
+static int k_twist(const Geo& g, int prec, VecArg out, VecArg in, double c0, double c1, int nrhs, cudaStream_t st)
+{
+    dim3 grid(blas_blocks(g.Vh), nrhs);
+    return by_prec(prec, [&](auto P) {
+        twist_kernel<decltype(P)::value><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, out, in, c0, c1);
+        TM_LAUNCH_CHECK("twist_kernel");
+        return (int)TM_OK;
+    });
+}
+
+template <int FIN>
+static int k_norm2(const Geo& g, int prec, VecArg v, const BlasCtx& c, int nrhs, cudaStream_t st)
+{
+    dim3 grid(blas_blocks(g.Vh), nrhs);
+    return by_prec(prec, [&](auto P) {
+        norm2_kernel<decltype(P)::value, FIN><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, v, c);
+        TM_LAUNCH_CHECK("norm2_kernel");
+        return (int)TM_OK;
+    });
+}
+
+// out(po) = in(pi) [and out2]
+static int k_convert(const Geo& g, int po, int pi, VecArg out, VecArg out2, VecArg in, int nrhs, cudaStream_t st)
+{
+    dim3 grid(blas_blocks(g.Vh), nrhs);
+    return by_prec(po, [&](auto PO) {
+        return by_prec(pi, [&](auto PI) {
+            convert_kernel<decltype(PO)::value, decltype(PI)::value><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, out, out2, in);
+            TM_LAUNCH_CHECK("convert_kernel");
+            return (int)TM_OK;
+        });
+    });
+}
+
+template <int REDUCE>
+static int k_axpby(const Geo& g, int py, int px, VecArg y, VecArg x, double a, double b, const BlasCtx& c, int nrhs, cudaStream_t st)
+{
+    dim3 grid(blas_blocks(g.Vh), nrhs);
+    return by_prec(py, [&](auto PY) {
+        return by_prec(px, [&](auto PX) {
+            axpby_kernel<decltype(PY)::value, decltype(PX)::value, REDUCE><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, y, x, a, b, c);
+            TM_LAUNCH_CHECK("axpby_kernel");
+            return (int)TM_OK;
+        });
+    });
+}
+
+static int k_cg_iter(const Geo& g, const void* gauge, int prec, int recon, VecArg x, VecArg r, VecArg p, VecArg Ap, void* tmp,
+                     double kappa, double mu, const BlasCtx& c, int nrhs, bool do_update_p, cudaStream_t st)
+{
+    int rc = mdagm_apply(g, gauge, prec, recon, Ap.p, Ap.stride, p.p, p.stride, tmp, 0, kappa, mu, nrhs, c.active, st);
+    if (rc != TM_OK) return rc;
+    dim3 grid(blas_blocks(g.Vh), nrhs);
+    return by_prec(prec, [&](auto P) {
+        constexpr int PR = decltype(P)::value;
+        dot_pAp_kernel<PR><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, p, Ap, c);
+        TM_LAUNCH_CHECK("dot_pAp_kernel");
+        update_xr_kernel<PR><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, x, r, p, Ap, c);
+        TM_LAUNCH_CHECK("update_xr_kernel");
+        if (do_update_p) {
+            update_p_kernel<PR><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, p, r, c);
+            TM_LAUNCH_CHECK("update_p_kernel");
+        }
+        return (int)TM_OK;
+    });
+}
+
+static int k_update_p(const Geo& g, int prec, VecArg p, VecArg r, const BlasCtx& c, int nrhs, cudaStream_t st)
+{
+    dim3 grid(blas_blocks(g.Vh), nrhs);
+    return by_prec(prec, [&](auto P) {
+        update_p_kernel<decltype(P)::value><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, p, r, c);
+        TM_LAUNCH_CHECK("update_p_kernel");
+        return (int)TM_OK;
+    });
+}
+
+// carve a workspace
+struct Carver {
+    char* base;
+    size_t off = 0, cap;
+    Carver(void* p, size_t c) : base(static_cast<char*>(p)), cap(c) {}
+    void* take(size_t n)
+    {
+        void* r = base + off;
+        off += round256(n);
+        return r;
+    }
+    bool ok() const { return off <= cap; }
+};
+
+static size_t ctx_bytes(int nrhs)
+{
+    return round256(sizeof(CgScal) * nrhs) + round256(nrhs) + round256(sizeof(unsigned int) * nrhs) +
+           round256(sizeof(double) * BLAS_MAX_BLOCKS * nrhs);
+}
+
+static BlasCtx carve_ctx(Carver& cv, int nrhs)
+{
+    BlasCtx c;
+    c.scal = static_cast<CgScal*>(cv.take(sizeof(CgScal) * nrhs));
+    c.active = static_cast<unsigned char*>(cv.take(nrhs));
+    c.tickets = static_cast<unsigned int*>(cv.take(sizeof(unsigned int) * nrhs));
+    c.partials = static_cast<double*>(cv.take(sizeof(double) * BLAS_MAX_BLOCKS * nrhs));
+    return c;
+}
+
+static int init_ctx(const BlasCtx& c, const tm_cg_params* p, int nrhs, cudaStream_t st)
+{
+    std::vector<CgScal> h(nrhs);
+    for (auto& s : h) {
+        memset(&s, 0, sizeof(s));
+        s.tol2 = p->tol * p->tol;
+        s.max_iter = p->max_iter;
+        s.status = TM_ERR_MAXITER;
+    }
+    TM_CUDA_CHECK(cudaMemcpyAsync(c.scal, h.data(), sizeof(CgScal) * nrhs, cudaMemcpyHostToDevice, st));
+    TM_CUDA_CHECK(cudaMemsetAsync(c.active, 1, nrhs, st));
+    TM_CUDA_CHECK(cudaMemsetAsync(c.tickets, 0, sizeof(unsigned int) * nrhs, st));
+    TM_CUDA_CHECK(cudaStreamSynchronize(st)); // h goes out of scope
+    return TM_OK;
+}
+
+// b'' (stride pb) from the full-lattice source; t1, t2: scratch (stride pb)
+static int prepare_rhs(const Geo& g, const void* gauge, int prec, int recon, const void* eta_full, void* b, void* t1, void* t2,
+                       double kappa, double mu, int nrhs, cudaStream_t st)
+{
+    const size_t pb = spinor_parity_bytes(g, prec);
+    const char* eta_e = static_cast<const char*>(eta_full);
+    const char* eta_o = eta_e + pb;
+    const double a = 2.0 * kappa * mu, n = 1.0 / (1.0 + a * a);
+    int rc;
+    // t1 = R^-1 eta_o
+    if ((rc = k_twist(g, prec, V_(t1, pb), V_(eta_o, 2 * pb), n, -a * n, nrhs, st)) != TM_OK) return rc;
+    DslashParams p;
+    p.gauge = gauge; p.nrhs = nrhs; p.active = nullptr;
+    // t2 = b' = eta_e + kappa D_eo t1
+    p.out = t2; p.in = t1; p.x = eta_e; p.out_parity = 0; p.dagger = 0;
+    p.rhs_stride_out = pb; p.rhs_stride_in = pb; p.rhs_stride_x = 2 * pb;
+    p.pq[0] = 1.0; p.pq[1] = 0.0; p.pq[2] = kappa; p.pq[3] = 0.0;
+    if ((rc = launch_dslash(g, prec, recon, p, st)) != TM_OK) return rc;
+    // t1 = R(-a)^-1 D^dag_oe b'
+    p.out = t1; p.in = t2; p.x = nullptr; p.out_parity = 1; p.dagger = 1; p.rhs_stride_x = pb;
+    kind_pq(TM_KIND_TWIST_INV, 1, kappa, mu, p.pq);
+    if ((rc = launch_dslash(g, prec, recon, p, st)) != TM_OK) return rc;
+    // b = R(-a) b' - kappa^2 D^dag_eo t1
+    p.out = b; p.in = t1; p.x = t2; p.out_parity = 0;
+    kind_pq(TM_KIND_XPAY_TWIST, 1, kappa, mu, p.pq);
+    return launch_dslash(g, prec, recon, p, st);
+}
+
+// s_o = R^-1 eta_o + kappa R^-1 D_oe s_e   (all inside the full-lattice arrays, stride 2 pb)
+static int reconstruct_odd(const Geo& g, const void* gauge, int prec, int recon, void* s_full, const void* eta_full, double kappa,
+                           double mu, int nrhs, cudaStream_t st)
+{
+    const size_t pb = spinor_parity_bytes(g, prec);
+    const double a = 2.0 * kappa * mu, n = 1.0 / (1.0 + a * a);
+    DslashParams p;
+    p.gauge = gauge; p.nrhs = nrhs; p.active = nullptr;
+    p.out = static_cast<char*>(s_full) + pb; p.in = s_full; p.x = static_cast<const char*>(eta_full) + pb;
+    p.out_parity = 1; p.dagger = 0;
+    p.rhs_stride_out = p.rhs_stride_in = p.rhs_stride_x = 2 * pb;
+    p.pq[0] = n; p.pq[1] = -a * n; p.pq[2] = kappa * n; p.pq[3] = -kappa * a * n;
+    return launch_dslash(g, prec, recon, p, st);
+}
+
+size_t cg_lp_workspace_bytes(const Geo& g, int prec, int nrhs)
+{
+    return ctx_bytes(nrhs) + 6 * round256(spinor_parity_bytes(g, prec) * nrhs);
+}
+
+// truncated LP solve, batched
+int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* s_full, const void* eta_full,
+                    const tm_cg_params* prm, int nrhs, tm_cg_info* info, void* ws, size_t ws_bytes, cudaStream_t st)
+{
+    const size_t pb = spinor_parity_bytes(g, prec);
+    Carver cv(ws, ws_bytes);
+    BlasCtx c = carve_ctx(cv, nrhs);
+    void* b = cv.take(pb * nrhs);
+    void* r = cv.take(pb * nrhs);
+    void* p = cv.take(pb * nrhs);
+    void* Ap = cv.take(pb * nrhs);
+    void* t1 = cv.take(2 * pb * nrhs); // t1, t2 contiguous (mdagm_apply tmp)
+    void* t2 = static_cast<char*>(t1) + pb * nrhs;
+    if (!cv.ok()) return TM_ERR_LAYOUT;
+    int rc;
+    if ((rc = init_ctx(c, prm, nrhs, st)) != TM_OK) return rc;
+    if ((rc = prepare_rhs(g, gauge, prec, recon, eta_full, b, t1, t2, prm->kappa, prm->mu, nrhs, st)) != TM_OK) return rc;
+    if ((rc = k_norm2<FIN_INIT>(g, prec, V_(b, pb), c, nrhs, st)) != TM_OK) return rc;
+    if ((rc = k_convert(g, prec, prec, V_(r, pb), V_(p, pb), V_(b, pb), nrhs, st)) != TM_OK) return rc;
+    VecArg x = V_(s_full, 2 * pb); // s_e lives in the even block of s_full
+    TM_CUDA_CHECK(cudaMemset2DAsync(s_full, 2 * pb, 0, pb, nrhs, st));
+    const int every = prm->check_every > 0 ? prm->check_every : 4;
+    unsigned char hact[TM_MAX_NRHS];
+    for (int k = 0; k < prm->max_iter;) {
+        for (int j = 0; j < every && k < prm->max_iter; ++j, ++k)
+            if ((rc = k_cg_iter(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), V_(Ap, pb), t1, prm->kappa, prm->mu, c, nrhs, true,
+                                st)) != TM_OK)
+                return rc;
+        TM_CUDA_CHECK(cudaMemcpyAsync(hact, c.active, nrhs, cudaMemcpyDeviceToHost, st));
+        TM_CUDA_CHECK(cudaStreamSynchronize(st));
+        bool any = false;
+        for (int q = 0; q < nrhs; ++q) any |= hact[q] != 0;
+        if (!any) break;
+    }
+    if ((rc = reconstruct_odd(g, gauge, prec, recon, s_full, eta_full, prm->kappa, prm->mu, nrhs, st)) != TM_OK) return rc;
+    // recomputed residual of the normal system, in the same storage/arithmetic: Ap = A x; Ap = b - Ap
+    if ((rc = mdagm_apply(g, gauge, prec, recon, Ap, pb, s_full, 2 * pb, t1, 0, prm->kappa, prm->mu, nrhs, nullptr, st)) != TM_OK) return rc;
+    if ((rc = k_axpby<1>(g, prec, prec, V_(Ap, pb), V_(b, pb), -1.0, 1.0, c, nrhs, st)) != TM_OK) return rc;
+    std::vector<CgScal> h(nrhs);
+    TM_CUDA_CHECK(cudaMemcpyAsync(h.data(), c.scal, sizeof(CgScal) * nrhs, cudaMemcpyDeviceToHost, st));
+    TM_CUDA_CHECK(cudaStreamSynchronize(st));
+    int worst = TM_OK;
+    for (int q = 0; q < nrhs; ++q) {
+        info[q].iters = h[q].iter;
+        info[q].status = h[q].status;
+        info[q].reliable_updates = 0;
+        info[q].iterated_resid = h[q].b2 > 0 ? std::sqrt(h[q].rr / h[q].b2) : 0.0;
+        info[q].true_resid = h[q].b2 > 0 ? std::sqrt(h[q].aux / h[q].b2) : 0.0;
+        if (h[q].b2 == 0.0) info[q].status = TM_OK;
+        if (info[q].status == TM_ERR_MAXITER && prm->tol == 0.0) info[q].status = TM_OK; // fixed-iteration truncation
+        if (info[q].status != TM_OK && (worst == TM_OK || info[q].status == TM_ERR_BREAKDOWN)) worst = info[q].status;
+    }
+    return worst;
+}
+
+} // namespace tmk
+
+namespace tmk {
+
+size_t cg_hp_workspace_bytes(const Geo& g, int prec_hp, int prec_lp)
+{
+    return ctx_bytes(1) + 4 * round256(spinor_parity_bytes(g, prec_hp)) + 6 * round256(spinor_parity_bytes(g, prec_lp));
+}
+
+static int read_scal(const BlasCtx& c, CgScal* h, cudaStream_t st)
+{
+    TM_CUDA_CHECK(cudaMemcpyAsync(h, c.scal, sizeof(CgScal), cudaMemcpyDeviceToHost, st));
+    TM_CUDA_CHECK(cudaStreamSynchronize(st));
+    return TM_OK;
+}
+
+static int write_scal(const BlasCtx& c, const CgScal* h, unsigned char active, cudaStream_t st)
+{
+    TM_CUDA_CHECK(cudaMemcpyAsync(c.scal, h, sizeof(CgScal), cudaMemcpyHostToDevice, st));
+    TM_CUDA_CHECK(cudaMemsetAsync(c.active, active, 1, st));
+    TM_CUDA_CHECK(cudaStreamSynchronize(st));
+    return TM_OK;
+}
+
+// mixed-precision solve of ONE right-hand side: CG iterations in prec_lp, reliable updates in prec_hp
+// (reading 10).  eta_full / s_full are packed at prec_hp.
+int cg_hp_mixed(const Geo& g, const void* gauge_hp, int prec_hp, const void* gauge_lp, int prec_lp, int recon, void* s_full,
+                const void* eta_full, const tm_cg_params* prm, tm_cg_info* info, void* ws, size_t ws_bytes, cudaStream_t st)
+{
+    const size_t pbh = spinor_parity_bytes(g, prec_hp), pbl = spinor_parity_bytes(g, prec_lp);
+    Carver cv(ws, ws_bytes);
+    BlasCtx c = carve_ctx(cv, 1);
+    void* b = cv.take(pbh);
+    void* rh = cv.take(pbh);
+    void* th = cv.take(2 * pbh);
+    void* r = cv.take(pbl);
+    void* p = cv.take(pbl);
+    void* Ap = cv.take(pbl);
+    void* xl = cv.take(pbl);
+    void* tl = cv.take(2 * pbl);
+    if (!cv.ok()) return TM_ERR_LAYOUT;
+    const double kappa = prm->kappa, mu = prm->mu;
+    const double delta = prm->reliable_delta > 0 ? prm->reliable_delta : 0.1;
+    int rc;
+    if ((rc = init_ctx(c, prm, 1, st)) != TM_OK) return rc;
+    if ((rc = prepare_rhs(g, gauge_hp, prec_hp, recon, eta_full, b, th, static_cast<char*>(th) + pbh, kappa, mu, 1, st)) != TM_OK) return rc;
+    if ((rc = k_norm2<FIN_INIT>(g, prec_hp, V_(b, pbh), c, 1, st)) != TM_OK) return rc;
+    if ((rc = k_convert(g, prec_lp, prec_hp, V_(r, pbl), V_(p, pbl), V_(b, pbh), 1, st)) != TM_OK) return rc;
+    TM_CUDA_CHECK(cudaMemsetAsync(s_full, 0, pbh, st)); // x_hp = s_e = 0
+    TM_CUDA_CHECK(cudaMemsetAsync(xl, 0, pbl, st));
+    CgScal h;
+    if ((rc = read_scal(c, &h, st)) != TM_OK) return rc;
+    const double b2 = h.b2;
+    info->iters = 0; info->reliable_updates = 0; info->status = TM_OK; info->iterated_resid = 0; info->true_resid = 0;
+    if (!(b2 > 0.0)) {
+        TM_CUDA_CHECK(cudaMemsetAsync(s_full, 0, 2 * pbh, st));
+        return reconstruct_odd(g, gauge_hp, prec_hp, recon, s_full, eta_full, kappa, mu, 1, st);
+    }
+    // the LP iteration never decides convergence on its own: tol2 = 0 on the device, the host decides
+    h.tol2 = 0.0;
+    if ((rc = write_scal(c, &h, 1, st)) != TM_OK) return rc;
+    double rr_prev = h.rr, rr_max = h.rr, rr_true = h.rr;
+    const double target2 = prm->tol * prm->tol * b2;
+    int status = TM_ERR_MAXITER;
+    bool x_dirty = false;
+    int k = 0;
+    while (k < prm->max_iter) {
+        if ((rc = k_cg_iter(g, gauge_lp, prec_lp, recon, V_(xl, pbl), V_(r, pbl), V_(p, pbl), V_(Ap, pbl), tl, kappa, mu, c, 1, false,
+                            st)) != TM_OK)
+            return rc;
+        ++k;
+        x_dirty = true;
+        if ((rc = read_scal(c, &h, st)) != TM_OK) return rc;
+        if (h.status == TM_ERR_BREAKDOWN) { status = TM_ERR_BREAKDOWN; break; }
+        const double rr = h.rr;
+        if (rr > rr_max) rr_max = rr;
+        const bool want = (rr < delta * delta * rr_max) || (rr <= target2) || (k == prm->max_iter);
+        if (want) {
+            // x_hp += x_lp; x_lp = 0; r_hp = b - A_hp x_hp
+            if ((rc = k_axpby<0>(g, prec_hp, prec_lp, V_(s_full, 2 * pbh), V_(xl, pbl), 1.0, 1.0, c, 1, st)) != TM_OK) return rc;
+            TM_CUDA_CHECK(cudaMemsetAsync(xl, 0, pbl, st));
+            x_dirty = false;
+            if ((rc = mdagm_apply(g, gauge_hp, prec_hp, recon, rh, pbh, s_full, 2 * pbh, th, 0, kappa, mu, 1, nullptr, st)) != TM_OK) return rc;
+            if ((rc = k_axpby<1>(g, prec_hp, prec_hp, V_(rh, pbh), V_(b, pbh), -1.0, 1.0, c, 1, st)) != TM_OK) return rc;
+            if ((rc = k_convert(g, prec_lp, prec_hp, V_(r, pbl), V_((void*)nullptr, 0), V_(rh, pbh), 1, st)) != TM_OK) return rc;
+            if ((rc = read_scal(c, &h, st)) != TM_OK) return rc;
+            rr_true = h.aux;
+            info->reliable_updates += 1;
+            info->iterated_resid = std::sqrt(rr / b2);
+            if (rr_true <= target2) { status = TM_OK; break; }
+            h.rr = rr_true;
+            h.beta = rr_true / rr_prev;
+            h.status = TM_ERR_MAXITER;
+            if ((rc = write_scal(c, &h, 1, st)) != TM_OK) return rc;
+            rr_max = rr_true;
+            rr_prev = rr_true;
+        } else {
+            rr_prev = rr;
+            info->iterated_resid = std::sqrt(rr / b2);
+        }
+        if (k < prm->max_iter)
+            if ((rc = k_update_p(g, prec_lp, V_(p, pbl), V_(r, pbl), c, 1, st)) != TM_OK) return rc;
+    }
+    (void)x_dirty;
+    info->iters = k;
+    info->status = status;
+    info->true_resid = std::sqrt(rr_true / b2);
+    if ((rc = reconstruct_odd(g, gauge_hp, prec_hp, recon, s_full, eta_full, kappa, mu, 1, st)) != TM_OK) return rc;
+    TM_CUDA_CHECK(cudaStreamSynchronize(st));
+    return status;
+}
+
+} // namespace tmk
+
+using namespace tmk;
+
+extern "C" size_t tm_cg_workspace_bytes(const tm_lattice* L, int prec_hp, int prec_lp, int mode, int nrhs)
+{
+    if (!L || !valid_prec(prec_lp) || nrhs < 1 || nrhs > TM_MAX_NRHS) return 0;
+    if (mode == TM_CG_LP_TRUNCATED) return cg_lp_workspace_bytes(L->g, prec_lp, nrhs);
+    if (!valid_prec(prec_hp)) return 0;
+    return cg_hp_workspace_bytes(L->g, prec_hp, prec_lp);
+}
+
+extern "C" int tm_cg_multi(const tm_lattice* L, const void* gauge_hp, int prec_hp, const void* gauge_lp, int prec_lp, int recon,
+                           void* s_full, const void* eta_full, const tm_cg_params* p, int nrhs, tm_cg_info* info, void* workspace,
+                           size_t workspace_bytes, void* stream)
+{
+    if (!L || !gauge_lp || !s_full || !eta_full || !p || !info || !workspace) return TM_ERR_ARG;
+    if (!valid_prec(prec_lp) || !valid_recon(recon) || nrhs < 1 || nrhs > TM_MAX_NRHS || p->max_iter < 0 || p->tol < 0) return TM_ERR_ARG;
+    if (!aligned256(gauge_lp) || !aligned256(s_full) || !aligned256(eta_full) || !aligned256(workspace)) return TM_ERR_LAYOUT;
+    if (workspace_bytes < tm_cg_workspace_bytes(L, prec_hp, prec_lp, p->mode, nrhs)) return TM_ERR_LAYOUT;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (p->mode == TM_CG_LP_TRUNCATED)
+        return cg_lp_truncated(L->g, gauge_lp, prec_lp, recon, s_full, eta_full, p, nrhs, info, workspace, workspace_bytes, st);
+    if (p->mode != TM_CG_HP_MIXED || !gauge_hp || !valid_prec(prec_hp) || !aligned256(gauge_hp)) return TM_ERR_ARG;
+    // HP_MIXED: right-hand sides are solved one after the other (reliable-update decisions are per solve)
+    const size_t fb = 2 * spinor_parity_bytes(L->g, prec_hp);
+    int worst = TM_OK;
+    for (int q = 0; q < nrhs; ++q) {
+        const int rc = cg_hp_mixed(L->g, gauge_hp, prec_hp, gauge_lp, prec_lp, recon, static_cast<char*>(s_full) + q * fb,
+                                   static_cast<const char*>(eta_full) + q * fb, p, info + q, workspace, workspace_bytes, st);
+        if (rc == TM_ERR_CUDA || rc == TM_ERR_LAYOUT) return rc;
+        if (rc != TM_OK && (worst == TM_OK || rc == TM_ERR_BREAKDOWN)) worst = rc;
+    }
+    return worst;
+}
+
+extern "C" int tm_cg(const tm_lattice* L, const void* gauge_hp, int prec_hp, const void* gauge_lp, int prec_lp, int recon,
+                     void* s_full, const void* eta_full, const tm_cg_params* p, tm_cg_info* info, void* workspace,
+                     size_t workspace_bytes, void* stream)
+{
+    return tm_cg_multi(L, gauge_hp, prec_hp, gauge_lp, prec_lp, recon, s_full, eta_full, p, 1, info, workspace, workspace_bytes, stream);
+}
+
+extern "C" size_t tm_tsm_workspace_bytes(const tm_lattice* L, int prec_lp, int nrhs)
+{
+    if (!L || !valid_prec(prec_lp) || nrhs < 1 || nrhs > TM_MAX_NRHS) return 0;
+    const size_t fb = 2 * spinor_parity_bytes(L->g, prec_lp) * nrhs;
+    return round256((size_t)L->V * 12 * nrhs) + 2 * round256(fb) + cg_lp_workspace_bytes(L->g, prec_lp, nrhs) +
+           loop_workspace_bytes(L->g, nrhs) + round256((size_t)nrhs * 16 * L->g.T * 2 * sizeof(double));
+}
+
+extern "C" int tm_tsm_batch_host(const tm_lattice* L, const void* gauge_lp, int prec_lp, int recon, const unsigned char* codes_host,
+                                 const tm_cg_params* p, int nrhs, tm_cg_info* info, double* loops_host, void* workspace,
+                                 size_t workspace_bytes, void* stream)
+{
+    if (!L || !gauge_lp || !codes_host || !p || !info || !loops_host || !workspace) return TM_ERR_ARG;
+    if (!valid_prec(prec_lp) || !valid_recon(recon) || nrhs < 1 || nrhs > TM_MAX_NRHS) return TM_ERR_ARG;
+    if (!aligned256(gauge_lp) || !aligned256(workspace)) return TM_ERR_LAYOUT;
+    if (workspace_bytes < tm_tsm_workspace_bytes(L, prec_lp, nrhs)) return TM_ERR_LAYOUT;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geo& g = L->g;
+    const size_t fb = 2 * spinor_parity_bytes(g, prec_lp) * nrhs;
+    Carver cv(workspace, workspace_bytes);
+    unsigned char* codes = static_cast<unsigned char*>(cv.take((size_t)L->V * 12 * nrhs));
+    void* eta = cv.take(fb);
+    void* s = cv.take(fb);
+    const size_t cgb = cg_lp_workspace_bytes(g, prec_lp, nrhs);
+    void* cgws = cv.take(cgb);
+    void* lws = cv.take(loop_workspace_bytes(g, nrhs));
+    const size_t lb = (size_t)nrhs * 16 * g.T * 2 * sizeof(double);
+    double* loops = static_cast<double*>(cv.take(lb));
+    if (!cv.ok()) return TM_ERR_LAYOUT;
+    TM_CUDA_CHECK(cudaMemcpyAsync(codes, codes_host, (size_t)L->V * 12 * nrhs, cudaMemcpyHostToDevice, st));
+    int rc = spinor_pack_any(g, L->V, prec_lp, 2, nullptr, nullptr, codes, eta, nrhs, st);
+    if (rc != TM_OK) return rc;
+    tm_cg_params q = *p;
+    q.mode = TM_CG_LP_TRUNCATED;
+    const int rc_cg = cg_lp_truncated(g, gauge_lp, prec_lp, recon, s, eta, &q, nrhs, info, cgws, cgb, st);
+    if (rc_cg == TM_ERR_CUDA || rc_cg == TM_ERR_LAYOUT) return rc_cg;
+    if ((rc = loop_contract(g, eta, s, prec_lp, nrhs, loops, lws, st)) != TM_OK) return rc;
+    TM_CUDA_CHECK(cudaMemcpyAsync(loops_host, loops, lb, cudaMemcpyDeviceToHost, st));
+    TM_CUDA_CHECK(cudaStreamSynchronize(st));
+    return rc_cg;
+}

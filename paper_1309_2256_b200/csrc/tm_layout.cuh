@@ -1,0 +1,180 @@
+// tm_layout.cuh -- packed device layout: even-odd structure of arrays in 16-byte chunks.
+//
+// One-parity spinor, Vh sites, checkerboard index cb:
+//   real r = (spin*3 + colour)*2 + reim, r = 0..23
+//   fp64: 12 chunks of double2  -> chunk k holds reals 2k, 2k+1       at ((double2*)base)[k*Vh + cb]
+//   fp32:  6 chunks of float4   -> chunk k holds reals 4k..4k+3       at ((float4*)base)[k*Vh + cb]
+//   fp16:  3 chunks of 8 halves -> chunk k holds reals 8k..8k+7       at ((uint4*)base)[k*Vh + cb]
+//          followed by Vh fp32 norms; value = half * norm, norm = max |real| of the site (north_star:
+//          "fp16 storage with a per-site fp32 norm").
+// One (parity, mu) link block, R = 18 or 12 reals per link, real r = (row*3 + col)*2 + reim:
+//   fp64: R/2 chunks of double2
+//   fp32: 18 -> 4 float4 chunks + 1 float2 tail array; 12 -> 3 float4 chunks
+//   fp16: 18 -> 2 uint4 chunks + 1 half2 (4-byte) tail array; 12 -> 1 uint4 chunk + 1 uint2 (8-byte) tail array
+// Links are stored unscaled (|U_ij| <= 1).  With R = 12 the third row is rebuilt as conj(row0 x row1)
+// ("12-parameter reconstruction").
+#pragma once
+#include "tm_common.cuh"
+
+namespace tmk {
+
+template <int PREC> struct Prec;
+template <> struct Prec<8> { typedef double real; };
+template <> struct Prec<4> { typedef float real; };
+template <> struct Prec<2> { typedef float real; };
+
+__device__ __forceinline__ uint4 ldg128(const void* p) { return __ldg(reinterpret_cast<const uint4*>(p)); }
+__device__ __forceinline__ uint2 ldg64(const void* p) { return __ldg(reinterpret_cast<const uint2*>(p)); }
+__device__ __forceinline__ uint32_t ldg32(const void* p) { return __ldg(reinterpret_cast<const uint32_t*>(p)); }
+
+__device__ __forceinline__ void unpack_h2(uint32_t w, float& a, float& b)
+{
+    const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&w));
+    a = f.x;
+    b = f.y;
+}
+__device__ __forceinline__ uint32_t pack_h2(float a, float b)
+{
+    const __half2 h = __floats2half2_rn(a, b);
+    return *reinterpret_cast<const uint32_t*>(&h);
+}
+
+// ------------------------------------------------------------------------------------------------
+// spinor load: v[24] in arithmetic precision
+// ------------------------------------------------------------------------------------------------
+template <int PREC>
+__device__ __forceinline__ void load_spinor(const void* base, int Vh, int cb, typename Prec<PREC>::real* v)
+{
+    if constexpr (PREC == 8) {
+        const double2* p = reinterpret_cast<const double2*>(base) + cb;
+#pragma unroll
+        for (int k = 0; k < 12; ++k) {
+            const double2 d = __ldg(p + (size_t)k * Vh);
+            v[2 * k] = d.x;
+            v[2 * k + 1] = d.y;
+        }
+    } else if constexpr (PREC == 4) {
+        const float4* p = reinterpret_cast<const float4*>(base) + cb;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            const float4 d = __ldg(p + (size_t)k * Vh);
+            v[4 * k] = d.x;
+            v[4 * k + 1] = d.y;
+            v[4 * k + 2] = d.z;
+            v[4 * k + 3] = d.w;
+        }
+    } else {
+        const uint4* p = reinterpret_cast<const uint4*>(base) + cb;
+        uint4 q[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) q[k] = __ldg(p + (size_t)k * Vh);
+        const float nrm = __ldg(reinterpret_cast<const float*>(reinterpret_cast<const uint4*>(base) + (size_t)3 * Vh) + cb);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            unpack_h2(q[k].x, v[8 * k + 0], v[8 * k + 1]);
+            unpack_h2(q[k].y, v[8 * k + 2], v[8 * k + 3]);
+            unpack_h2(q[k].z, v[8 * k + 4], v[8 * k + 5]);
+            unpack_h2(q[k].w, v[8 * k + 6], v[8 * k + 7]);
+        }
+#pragma unroll
+        for (int r = 0; r < 24; ++r) v[r] *= nrm;
+    }
+}
+
+template <int PREC>
+__device__ __forceinline__ void store_spinor(void* base, int Vh, int cb, const typename Prec<PREC>::real* v)
+{
+    if constexpr (PREC == 8) {
+        double2* p = reinterpret_cast<double2*>(base) + cb;
+#pragma unroll
+        for (int k = 0; k < 12; ++k) p[(size_t)k * Vh] = make_double2(v[2 * k], v[2 * k + 1]);
+    } else if constexpr (PREC == 4) {
+        float4* p = reinterpret_cast<float4*>(base) + cb;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) p[(size_t)k * Vh] = make_float4(v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]);
+    } else {
+        float m = 0.f;
+#pragma unroll
+        for (int r = 0; r < 24; ++r) m = fmaxf(m, fabsf(v[r]));
+        const float inv = (m > 0.f) ? __fdividef(1.0f, m) : 0.f;
+        uint4* p = reinterpret_cast<uint4*>(base) + cb;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            uint4 q;
+            q.x = pack_h2(v[8 * k + 0] * inv, v[8 * k + 1] * inv);
+            q.y = pack_h2(v[8 * k + 2] * inv, v[8 * k + 3] * inv);
+            q.z = pack_h2(v[8 * k + 4] * inv, v[8 * k + 5] * inv);
+            q.w = pack_h2(v[8 * k + 6] * inv, v[8 * k + 7] * inv);
+            p[(size_t)k * Vh] = q;
+        }
+        reinterpret_cast<float*>(reinterpret_cast<uint4*>(base) + (size_t)3 * Vh)[cb] = m;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// link load: u[18] (row-major complex 3x3); RECON 12 rebuilds row 2
+// ------------------------------------------------------------------------------------------------
+template <typename real>
+__device__ __forceinline__ void rebuild_row2(real* u)
+{
+    // row2_j = conj(row0_{j+1} row1_{j+2} - row0_{j+2} row1_{j+1})
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const int j1 = (j + 1) % 3, j2 = (j + 2) % 3;
+        const real ar = u[2 * j1], ai = u[2 * j1 + 1], br = u[6 + 2 * j2], bi = u[6 + 2 * j2 + 1];
+        const real cr = u[2 * j2], ci = u[2 * j2 + 1], dr = u[6 + 2 * j1], di = u[6 + 2 * j1 + 1];
+        u[12 + 2 * j] = (ar * br - ai * bi) - (cr * dr - ci * di);
+        u[12 + 2 * j + 1] = -((ar * bi + ai * br) - (cr * di + ci * dr));
+    }
+}
+
+template <int PREC, int RECON>
+__device__ __forceinline__ void load_link(const void* block, int Vh, int cb, typename Prec<PREC>::real* u)
+{
+    if constexpr (PREC == 8) {
+        const double2* p = reinterpret_cast<const double2*>(block) + cb;
+#pragma unroll
+        for (int k = 0; k < RECON / 2; ++k) {
+            const double2 d = __ldg(p + (size_t)k * Vh);
+            u[2 * k] = d.x;
+            u[2 * k + 1] = d.y;
+        }
+    } else if constexpr (PREC == 4) {
+        const float4* p = reinterpret_cast<const float4*>(block) + cb;
+#pragma unroll
+        for (int k = 0; k < RECON / 4; ++k) {
+            const float4 d = __ldg(p + (size_t)k * Vh);
+            u[4 * k] = d.x;
+            u[4 * k + 1] = d.y;
+            u[4 * k + 2] = d.z;
+            u[4 * k + 3] = d.w;
+        }
+        if constexpr (RECON == 18) {
+            const float2 d = __ldg(reinterpret_cast<const float2*>(reinterpret_cast<const float4*>(block) + (size_t)4 * Vh) + cb);
+            u[16] = d.x;
+            u[17] = d.y;
+        }
+    } else {
+        const uint4* p = reinterpret_cast<const uint4*>(block) + cb;
+        constexpr int NC = RECON / 8; // 2 or 1 full chunks
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+            const uint4 q = __ldg(p + (size_t)k * Vh);
+            unpack_h2(q.x, u[8 * k + 0], u[8 * k + 1]);
+            unpack_h2(q.y, u[8 * k + 2], u[8 * k + 3]);
+            unpack_h2(q.z, u[8 * k + 4], u[8 * k + 5]);
+            unpack_h2(q.w, u[8 * k + 6], u[8 * k + 7]);
+        }
+        const void* tail = reinterpret_cast<const uint4*>(block) + (size_t)NC * Vh;
+        if constexpr (RECON == 18) {
+            unpack_h2(ldg32(reinterpret_cast<const uint32_t*>(tail) + cb), u[16], u[17]);
+        } else {
+            const uint2 q = ldg64(reinterpret_cast<const uint2*>(tail) + cb);
+            unpack_h2(q.x, u[8], u[9]);
+            unpack_h2(q.y, u[10], u[11]);
+        }
+    }
+    if constexpr (RECON == 12) rebuild_row2(u);
+}
+
+} // namespace tmk

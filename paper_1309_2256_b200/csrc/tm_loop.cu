@@ -1,0 +1,190 @@
+// tm_loop.cu -- a8 of SURVEY.md 8(a): per-time-slice stochastic loop contraction for the 16 Gamma_n.
+//
+//   L[n][t] = sum_{x: x4=t} a(x)^dag (Gamma_n x 1_colour) b(x)          (Eq. 10)
+// computed as the colour-traced Dirac-open 4x4 matrix C_{al be}(t) = sum_x sum_c conj(a_{al c}) b_{be c}
+// ("Traces were taken in color space, leaving the Dirac ... indices open ... a 4x4 matrix was
+// obtained, with enough information to reconstruct any arbitrary gamma insertion") followed by
+// L[n][t] = sum_{al be} (Gamma_n)_{al be} C_{al be}(t).
+// Time slice t of parity p is the contiguous checkerboard range [t*V3h, (t+1)*V3h).
+// Reduction: per-site products in the storage arithmetic (fp32 for fp32/fp16 inputs), accumulated in fp64 per
+// thread, warp shuffles, shared memory across warps, per-block partials, then one fixed-order final pass:
+// bit-reproducible, no floating-point atomics.
+#include "tm_layout.cuh"
+
+namespace tmk {
+
+struct GammaTable {
+    // Gamma_n has one non-zero entry per row: (Gamma_n)_{al, col[n][al]} = re + i im, entries in {+-1, +-i}
+    signed char col[16][4], re[16][4], im[16][4];
+};
+
+// own gamma table (chiral basis of include/tm.h), multiplied out in integer arithmetic on the host
+static GammaTable make_gamma_table()
+{
+    struct Z { int re, im; };
+    auto mul = [](Z a, Z b) { return Z{a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; };
+    Z g[4][4][4] = {};
+    // g_k = [[0, -i s_k], [i s_k, 0]], g_4 = [[0, 1], [1, 0]]
+    const Z s[3][2][2] = {{{{0, 0}, {1, 0}}, {{1, 0}, {0, 0}}}, {{{0, 0}, {0, -1}}, {{0, 1}, {0, 0}}}, {{{1, 0}, {0, 0}}, {{0, 0}, {-1, 0}}}};
+    for (int k = 0; k < 3; ++k)
+        for (int a = 0; a < 2; ++a)
+            for (int b = 0; b < 2; ++b) {
+                g[k][a][2 + b] = mul(Z{0, -1}, s[k][a][b]);
+                g[k][2 + a][b] = mul(Z{0, 1}, s[k][a][b]);
+            }
+    g[3][0][2] = g[3][1][3] = g[3][2][0] = g[3][3][1] = Z{1, 0};
+    GammaTable tb;
+    for (int n = 0; n < 16; ++n) {
+        Z p[4][4] = {};
+        for (int a = 0; a < 4; ++a) p[a][a] = Z{1, 0};
+        for (int k = 0; k < 4; ++k) {
+            if (!((n >> k) & 1)) continue;
+            Z q[4][4] = {};
+            for (int a = 0; a < 4; ++a)
+                for (int b = 0; b < 4; ++b)
+                    for (int c = 0; c < 4; ++c) {
+                        const Z m = mul(p[a][c], g[k][c][b]);
+                        q[a][b].re += m.re;
+                        q[a][b].im += m.im;
+                    }
+            for (int a = 0; a < 4; ++a)
+                for (int b = 0; b < 4; ++b) p[a][b] = q[a][b];
+        }
+        for (int a = 0; a < 4; ++a)
+            for (int b = 0; b < 4; ++b)
+                if (p[a][b].re != 0 || p[a][b].im != 0) {
+                    tb.col[n][a] = (signed char)b;
+                    tb.re[n][a] = (signed char)p[a][b].re;
+                    tb.im[n][a] = (signed char)p[a][b].im;
+                }
+    }
+    return tb;
+}
+
+constexpr int LOOP_THREADS = 128;
+
+template <int PREC>
+__global__ void __launch_bounds__(LOOP_THREADS) loop_partial_kernel(Geo g, const char* a_full, const char* b_full,
+                                                                    size_t parity_bytes, double* partial, int nb)
+{
+    typedef typename Prec<PREC>::real real;
+    const int t = blockIdx.y, rhs = blockIdx.z;
+    const char* af = a_full + (size_t)rhs * 2 * parity_bytes;
+    const char* bf = b_full + (size_t)rhs * 2 * parity_bytes;
+    double acc[32];
+#pragma unroll
+    for (int k = 0; k < 32; ++k) acc[k] = 0.0;
+    const int nsite = 2 * g.V3h;
+    for (int i = blockIdx.x * LOOP_THREADS + threadIdx.x; i < nsite; i += nb * LOOP_THREADS) {
+        const int parity = i >= g.V3h;
+        const int cb = t * g.V3h + (i - parity * g.V3h);
+        real a[24], b[24];
+        load_spinor<PREC>(af + parity * parity_bytes, g.Vh, cb, a);
+        load_spinor<PREC>(bf + parity * parity_bytes, g.Vh, cb, b);
+#pragma unroll
+        for (int al = 0; al < 4; ++al)
+#pragma unroll
+            for (int be = 0; be < 4; ++be) {
+                real re = 0, im = 0;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const real ar = a[(al * 3 + c) * 2], ai = a[(al * 3 + c) * 2 + 1];
+                    const real br = b[(be * 3 + c) * 2], bi = b[(be * 3 + c) * 2 + 1];
+                    re = fma(ar, br, re);
+                    re = fma(ai, bi, re);
+                    im = fma(ar, bi, im);
+                    im = fma(-ai, br, im);
+                }
+                acc[(al * 4 + be) * 2] += (double)re;
+                acc[(al * 4 + be) * 2 + 1] += (double)im;
+            }
+    }
+    __shared__ double sm[LOOP_THREADS / 32][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+        double v = acc[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (lane == 0) sm[warp][k] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double v = 0.0;
+#pragma unroll
+        for (int w = 0; w < LOOP_THREADS / 32; ++w) v += sm[w][threadIdx.x];
+        partial[(((size_t)rhs * g.T + t) * nb + blockIdx.x) * 32 + threadIdx.x] = v;
+    }
+}
+
+__global__ void loop_final_kernel(int T, int nb, const double* partial, GammaTable tb, double* out)
+{
+    const int t = blockIdx.x, rhs = blockIdx.y;
+    __shared__ double C[32];
+    if (threadIdx.x < 32) {
+        double v = 0.0;
+        const double* p = partial + ((size_t)rhs * T + t) * nb * 32 + threadIdx.x;
+        for (int b = 0; b < nb; ++b) v += p[(size_t)b * 32];
+        C[threadIdx.x] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 16) {
+        const int n = threadIdx.x;
+        double re = 0.0, im = 0.0;
+#pragma unroll
+        for (int al = 0; al < 4; ++al) {
+            const int be = tb.col[n][al];
+            const double gr = tb.re[n][al], gi = tb.im[n][al];
+            const double cr = C[(al * 4 + be) * 2], ci = C[(al * 4 + be) * 2 + 1];
+            re += gr * cr - gi * ci;
+            im += gr * ci + gi * cr;
+        }
+        out[(((size_t)rhs * 16 + n) * T + t) * 2] = re;
+        out[(((size_t)rhs * 16 + n) * T + t) * 2 + 1] = im;
+    }
+}
+
+static int loop_nb(const Geo& g)
+{
+    int nb = (2 * g.V3h) / (LOOP_THREADS * 16);
+    if (nb < 1) nb = 1;
+    if (nb > 32) nb = 32;
+    return nb;
+}
+
+int loop_contract(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,
+                  cudaStream_t st)
+{
+    static const GammaTable tb = make_gamma_table();
+    const int nb = loop_nb(g);
+    dim3 grid(nb, g.T, nrhs), block(LOOP_THREADS);
+    const size_t pb = spinor_parity_bytes(g, prec);
+    double* partial = static_cast<double*>(workspace);
+    if (prec == 8) loop_partial_kernel<8><<<grid, block, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, partial, nb);
+    else if (prec == 4) loop_partial_kernel<4><<<grid, block, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, partial, nb);
+    else loop_partial_kernel<2><<<grid, block, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, partial, nb);
+    TM_LAUNCH_CHECK("loop_partial_kernel");
+    loop_final_kernel<<<dim3(g.T, nrhs), 32, 0, st>>>(g.T, nb, partial, tb, out);
+    TM_LAUNCH_CHECK("loop_final_kernel");
+    return TM_OK;
+}
+
+size_t loop_workspace_bytes(const Geo& g, int nrhs) { return round256((size_t)nrhs * g.T * loop_nb(g) * 32 * sizeof(double)); }
+
+} // namespace tmk
+
+using namespace tmk;
+
+extern "C" size_t tm_loop_workspace_bytes(const tm_lattice* L, int nrhs)
+{
+    if (!L || nrhs < 1) return 0;
+    return loop_workspace_bytes(L->g, nrhs);
+}
+
+extern "C" int tm_loop_contract(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, double* out,
+                                void* workspace, void* stream)
+{
+    if (!L || !a_full || !b_full || !out || !workspace || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
+    if (!aligned256(a_full) || !aligned256(b_full) || !aligned256(out) || !aligned256(workspace)) return TM_ERR_LAYOUT;
+    return loop_contract(L->g, a_full, b_full, prec, nrhs, out, workspace, (cudaStream_t)stream);
+}

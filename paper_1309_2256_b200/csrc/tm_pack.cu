@@ -1,0 +1,187 @@
+// tm_pack.cu -- a0 / a1 of SURVEY.md 8(a): canonical fp64 fields <-> packed even-odd SoA at fp64/fp32/fp16.
+#include "tm_layout.cuh"
+
+namespace tmk {
+
+__device__ unsigned int g_su3_dev_bits; // max deviation from SU(3) seen by the last gauge pack (float bits)
+
+template <int PREC>
+__device__ __forceinline__ void store_reals(void* block, int Vh, int cb, const double* u, int n)
+{
+    // generic element-wise store following the chunk layout of tm_layout.cuh (n reals per site)
+    const int w = PREC;
+    const int bytes = n * w;
+    const int nfull = bytes / 16;      // 16-byte chunks
+    const int per = 16 / w;            // reals per full chunk
+    char* base = static_cast<char*>(block);
+    for (int r = 0; r < n; ++r) {
+        char* dst;
+        if (r < nfull * per) {
+            dst = base + ((size_t)(r / per) * Vh + cb) * 16 + (size_t)(r % per) * w;
+        } else {
+            const int tail_reals = n - nfull * per; // reals in the tail array
+            dst = base + (size_t)nfull * Vh * 16 + ((size_t)cb * tail_reals + (r - nfull * per)) * w;
+        }
+        if (PREC == 8) *reinterpret_cast<double*>(dst) = u[r];
+        else if (PREC == 4) *reinterpret_cast<float*>(dst) = (float)u[r];
+        else *reinterpret_cast<__half*>(dst) = __float2half_rn((float)u[r]);
+    }
+}
+
+template <int PREC, int RECON>
+__global__ void gauge_pack_kernel(Geo g, const double* __restrict__ U, char* out, size_t link_block, int check)
+{
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    const int pm = blockIdx.y; // parity*4 + mu
+    if (cb >= g.Vh) return;
+    const int parity = pm >> 2, mu = pm & 3;
+    uint32_t row, xh, rem2, y, t, z;
+    g.dXh.divmod((uint32_t)cb, row, xh);
+    g.dY.divmod(row, rem2, y);
+    g.dZ.divmod(rem2, t, z);
+    const int xodd = (parity + y + z + t) & 1;
+    const size_t site = 2 * (size_t)cb + xodd;
+    double u[18];
+#pragma unroll
+    for (int k = 0; k < 18; ++k) u[k] = U[(site * 4 + mu) * 18 + k];
+    if (check) {
+        // deviation from SU(3): |U U^dag - 1|_max and |row2 - conj(row0 x row1)|_max
+        double dev = 0;
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) {
+                double re = 0, im = 0;
+                for (int c = 0; c < 3; ++c) {
+                    const double ar = u[2 * (a * 3 + c)], ai = u[2 * (a * 3 + c) + 1];
+                    const double br = u[2 * (b * 3 + c)], bi = u[2 * (b * 3 + c) + 1];
+                    re += ar * br + ai * bi;
+                    im += ai * br - ar * bi;
+                }
+                dev = fmax(dev, fmax(fabs(re - (a == b ? 1.0 : 0.0)), fabs(im)));
+            }
+        double w[18];
+        for (int k = 0; k < 12; ++k) w[k] = u[k];
+        rebuild_row2(w);
+        for (int k = 12; k < 18; ++k) dev = fmax(dev, fabs(w[k] - u[k]));
+        if (!(dev == dev)) dev = 1e30; // NaN
+        atomicMax(&g_su3_dev_bits, __float_as_uint((float)dev));
+    }
+    store_reals<PREC>(out + (size_t)pm * link_block, g.Vh, cb, u, RECON);
+}
+
+template <int PREC, int MODE> // MODE 0: pack from fp64 canonical, 1: unpack to fp64 canonical, 2: pack from Z2xiZ2 codes
+__global__ void spinor_pack_kernel(Geo g, const double* __restrict__ src, double* dst, const unsigned char* __restrict__ codes,
+                                   char* packed, size_t parity_bytes, long long V)
+{
+    typedef typename Prec<PREC>::real real;
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    const int parity = blockIdx.y, rhs = blockIdx.z;
+    if (cb >= g.Vh) return;
+    uint32_t row, xh, rem2, y, t, z;
+    g.dXh.divmod((uint32_t)cb, row, xh);
+    g.dY.divmod(row, rem2, y);
+    g.dZ.divmod(rem2, t, z);
+    const int xodd = (parity + y + z + t) & 1;
+    const size_t site = (size_t)rhs * V + 2 * (size_t)cb + xodd;
+    char* field = packed + ((size_t)rhs * 2 + parity) * parity_bytes;
+    real v[24];
+    if (MODE == 0) {
+#pragma unroll
+        for (int k = 0; k < 24; ++k) v[k] = (real)src[site * 24 + k];
+        store_spinor<PREC>(field, g.Vh, cb, v);
+    } else if (MODE == 2) {
+        const real r = (real)0.70710678118654752440;
+#pragma unroll
+        for (int k = 0; k < 12; ++k) {
+            const unsigned c = codes[site * 12 + k];
+            v[2 * k] = (c & 1u) ? -r : r;
+            v[2 * k + 1] = (c & 2u) ? -r : r;
+        }
+        store_spinor<PREC>(field, g.Vh, cb, v);
+    } else {
+        load_spinor<PREC>(field, g.Vh, cb, v);
+#pragma unroll
+        for (int k = 0; k < 24; ++k) dst[site * 24 + k] = (double)v[k];
+    }
+}
+
+template <int PREC>
+static int gauge_pack_t(const Geo& g, const double* U, int recon, void* out, int check, cudaStream_t st)
+{
+    dim3 block(128), grid((g.Vh + 127) / 128, 8);
+    if (recon == 18) gauge_pack_kernel<PREC, 18><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 18), check);
+    else gauge_pack_kernel<PREC, 12><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 12), check);
+    TM_LAUNCH_CHECK("gauge_pack_kernel");
+    return TM_OK;
+}
+
+template <int PREC>
+static int spinor_pack_t(const Geo& g, long long V, int mode, const double* src, double* dst, const unsigned char* codes,
+                         void* packed, int nrhs, cudaStream_t st)
+{
+    dim3 block(128), grid((g.Vh + 127) / 128, 2, nrhs);
+    const size_t pb = spinor_parity_bytes(g, PREC);
+    if (mode == 0) spinor_pack_kernel<PREC, 0><<<grid, block, 0, st>>>(g, src, dst, codes, (char*)packed, pb, V);
+    else if (mode == 1) spinor_pack_kernel<PREC, 1><<<grid, block, 0, st>>>(g, src, dst, codes, (char*)packed, pb, V);
+    else spinor_pack_kernel<PREC, 2><<<grid, block, 0, st>>>(g, src, dst, codes, (char*)packed, pb, V);
+    TM_LAUNCH_CHECK("spinor_pack_kernel");
+    return TM_OK;
+}
+
+int spinor_pack_any(const Geo& g, long long V, int prec, int mode, const double* src, double* dst, const unsigned char* codes,
+                    void* packed, int nrhs, cudaStream_t st)
+{
+    if (prec == 8) return spinor_pack_t<8>(g, V, mode, src, dst, codes, packed, nrhs, st);
+    if (prec == 4) return spinor_pack_t<4>(g, V, mode, src, dst, codes, packed, nrhs, st);
+    return spinor_pack_t<2>(g, V, mode, src, dst, codes, packed, nrhs, st);
+}
+
+} // namespace tmk
+
+using namespace tmk;
+
+extern "C" int tm_gauge_pack(const tm_lattice* L, const double* U, int prec, int recon, void* out, double su3_tol, void* stream)
+{
+    if (!L || !U || !out || !valid_prec(prec) || !valid_recon(recon)) return TM_ERR_ARG;
+    if (!aligned256(U) || !aligned256(out)) return TM_ERR_LAYOUT;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int check = (recon == 12 && su3_tol > 0) ? 1 : 0;
+    if (check) {
+        const unsigned int zero = 0;
+        TM_CUDA_CHECK(cudaMemcpyToSymbolAsync(g_su3_dev_bits, &zero, sizeof(zero), 0, cudaMemcpyHostToDevice, st));
+    }
+    int rc;
+    if (prec == 8) rc = gauge_pack_t<8>(L->g, U, recon, out, check, st);
+    else if (prec == 4) rc = gauge_pack_t<4>(L->g, U, recon, out, check, st);
+    else rc = gauge_pack_t<2>(L->g, U, recon, out, check, st);
+    if (rc != TM_OK) return rc;
+    if (check) {
+        unsigned int bits = 0;
+        TM_CUDA_CHECK(cudaMemcpyFromSymbolAsync(&bits, g_su3_dev_bits, sizeof(bits), 0, cudaMemcpyDeviceToHost, st));
+        TM_CUDA_CHECK(cudaStreamSynchronize(st));
+        float dev;
+        memcpy(&dev, &bits, sizeof(dev));
+        if (dev > su3_tol) return TM_ERR_NOT_SU3;
+    }
+    return TM_OK;
+}
+
+extern "C" int tm_spinor_pack(const tm_lattice* L, const double* psi, int prec, int nrhs, void* out, void* stream)
+{
+    if (!L || !psi || !out || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
+    if (!aligned256(psi) || !aligned256(out)) return TM_ERR_LAYOUT;
+    return spinor_pack_any(L->g, L->V, prec, 0, psi, nullptr, nullptr, out, nrhs, (cudaStream_t)stream);
+}
+
+extern "C" int tm_spinor_unpack(const tm_lattice* L, const void* packed, int prec, int nrhs, double* psi, void* stream)
+{
+    if (!L || !psi || !packed || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
+    if (!aligned256(psi) || !aligned256(packed)) return TM_ERR_LAYOUT;
+    return spinor_pack_any(L->g, L->V, prec, 1, nullptr, psi, nullptr, const_cast<void*>(packed), nrhs, (cudaStream_t)stream);
+}
+
+extern "C" int tm_spinor_pack_z4(const tm_lattice* L, const unsigned char* codes, int prec, int nrhs, void* out, void* stream)
+{
+    if (!L || !codes || !out || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
+    if (!aligned256(codes) || !aligned256(out)) return TM_ERR_LAYOUT;
+    return spinor_pack_any(L->g, L->V, prec, 2, nullptr, nullptr, codes, out, nrhs, (cudaStream_t)stream);
+}
