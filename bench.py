@@ -1,0 +1,364 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the tm-dslash / MdagM / CG / loop library on B200.
+
+A "step" is one pass of the whole hot path over one batch of synthetic input at 32^3x64 (BASELINE.json
+configs[3], the paper's ensemble shape): 12 Z2xiZ2 noise sources -> pack -> batched truncated CG (tol 1e-2, fp16
+storage / fp32 arithmetic / fp64 reductions, 12-real links, every gauge load shared by the 12 right-hand sides) ->
+16-Gamma per-time-slice loop contraction of every solution.  metric = LP solves/s (BASELINE.json "LP solves/sec").
+The same run also reports BASELINE.json's other metric, single-RHS tm-dslash GFLOPS and algorithmic HBM GB/s at
+fp32 / fp16 x 18 / 12 reals (configs[2]), and a mixed-precision CG to 1e-8.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+N > 1: launched under torch.distributed.run; noise sources are independent, so ranks take different batches and
+there is no data-path collective (weak scaling, "replicas + gather" of the [16][T] loops).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+DIMS = (32, 32, 32, 64)
+NRHS = 12
+LP_TOL = 1e-2
+FLOPS_HOP, FLOPS_TWIST_INV, FLOPS_XPAY = 1320, 1392, 1416  # per output site
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12          # 148 SMs x 128 FP32 lanes x 2 (FMA) x max SM clock
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def cpu_oracle_sample():
+    """The oracle as it stands on the host cores: ONE complete truncated solve (tol 1e-2) + one 16-Gamma loop contraction on a
+    16^3x32 lattice (1/16 of the 32^3x64 sites, same generators/kappa/mu), scaled by the site ratio to solves/s at 32^3x64."""
+    import oracle
+    import tm_inputs as ti
+    dims = (16, 16, 16, 32)
+    U = ti.gauge(dims)
+    eta = ti.z4(dims)
+    t0 = time.time()
+    s, info = oracle.cg_solve(U, eta, ti.KAPPA, ti.MU, LP_TOL, 500)
+    oracle.loop(eta, s)
+    dt = time.time() - t0
+    scale = (32 ** 3 * 64) / (16 ** 3 * 32)
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    return {"value": 1.0 / (dt * scale), "unit": "solves/s", "cores": cores, "kind": "oracle",
+            "sample": "one truncated CG solve (tol 1e-2, %d iterations) + one 16-Gamma loop on 16^3x32 (1/16 of the sites) in %.1f s, "
+                      "scaled x1/16 to 32^3x64" % (info["iters"], dt)}, dt
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    vals, dts = [], []
+    base = None
+    for _ in range(args.steps):
+        base, dt = cpu_oracle_sample()
+        vals.append(base["value"]); dts.append(dt)
+    v = float(np.mean(vals))
+    base["value"] = v
+    print(json.dumps({
+        "impl": "reference", "metric": "LP solves/s", "value": v, "unit": "solves/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(dts)), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "32^3x64 TSM: truncated CG tol 1e-2 + 16-Gamma loop per source (oracle sample on 16^3x32, scaled)"},
+        "cpu_baseline": base, "e2e": {"value": v, "unit": "solves/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def dslash_bytes(Vh, prec, recon, has_x, nrhs=1):
+    """Minimal-traffic (algorithmic) bytes of one dslash launch: every link once, every input spinor once, output once
+    (+ x once); fp16 spinors carry a 4-byte norm."""
+    sp = 24 * prec + (4 if prec == 2 else 0)
+    return Vh * (8 * recon * prec + nrhs * (2 + (1 if has_x else 0)) * sp)
+
+
+def time_events(torch, fn, n):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(n):
+        fn(i)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / n
+
+
+def run_b200(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    import tm_inputs as ti
+    import paper_1309_2256_b200 as tm
+    tm.load()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    hbm_peak, peak_src = peaks()
+    L = tm.tm_lattice_create(DIMS, True)
+    V, Vh, T = L.V, L.V // 2, DIMS[3]
+    kappa, mu = ti.KAPPA, ti.MU
+
+    # ---- once per configuration: gauge field -> packed links (a0) ----
+    U = torch.from_numpy(ti.gauge(DIMS).view(np.float64)).cuda()
+    gauges = {}
+    for prec, recon in ((2, 12), (2, 18), (4, 12), (4, 18), (8, 12)):
+        gauges[(prec, recon)] = tm.device_buffer(tm.tm_gauge_bytes(L, prec, recon))
+        tm.tm_gauge_pack(L, U, prec, recon, gauges[(prec, recon)], 1e-10)
+    del U
+    torch.cuda.empty_cache()
+
+    # ---- inputs: two batches of 12 Z2xiZ2 sources per rank (302 MB each > L2), alternating ----
+    nb = 2
+    codes_host = [torch.from_numpy(np.stack([ti.z4_codes(DIMS, seed=ti.NOISE_SEED + (rank * nb + b) * NRHS + r) for r in range(NRHS)]))
+                  .pin_memory() for b in range(nb)]
+    codes_dev = [c.cuda() for c in codes_host]
+    prec, recon = 2, 12
+    g_lp = gauges[(prec, recon)]
+    fb = tm.tm_spinor_bytes(L, prec, 1, NRHS)
+    eta, sol = tm.device_buffer(fb), tm.device_buffer(fb)
+    cg_ws = tm.device_buffer(tm.tm_cg_workspace_bytes(L, 8, prec, tm.TM_CG_LP_TRUNCATED, NRHS))
+    loop_ws = tm.device_buffer(tm.tm_loop_workspace_bytes(L, NRHS))
+    loops = torch.zeros((NRHS, 16, T, 2), dtype=torch.float64, device="cuda")
+    tsm_ws = tm.device_buffer(tm.tm_tsm_workspace_bytes(L, prec, NRHS))
+    loops_host = torch.zeros((NRHS, 16, T, 2), dtype=torch.float64).pin_memory()
+    prm = tm.make_cg_params(kappa, mu, LP_TOL, 500, tm.TM_CG_LP_TRUNCATED, 0.1, 4)
+    iters_log = []
+
+    def step(i):
+        tm.tm_spinor_pack_z4(L, codes_dev[i % nb], prec, NRHS, eta)
+        rc, info = tm.tm_cg_multi(L, None, 8, g_lp, prec, recon, sol, eta, prm, NRHS, cg_ws)
+        assert rc == tm.TM_OK, rc
+        tm.tm_loop_contract(L, eta, sol, prec, NRHS, loops, loop_ws)
+        iters_log.append([x.iters for x in info])
+
+    def step_e2e(i):
+        rc, info = tm.tm_tsm_batch_host(L, g_lp, prec, recon, codes_host[i % nb], prm, NRHS, loops_host, tsm_ws)
+        assert rc == tm.TM_OK, rc
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---- warm-up, then EXACTLY K timed steps (device-resident inputs) ----
+    for i in range(args.warmup):
+        step(i)
+    iters_log.clear()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    tm.tm_kernel_timing_enable(1)
+    tm.tm_kernel_timing_read(True)
+    n0 = tm.tm_launch_count()
+    ms_step = time_events(torch, step, args.steps)
+    launches = tm.tm_launch_count() - n0
+    k_ms, k_n = tm.tm_kernel_timing_read(True)
+    tm.tm_kernel_timing_enable(0)
+    barrier()
+    clocks = sampler.stop()
+    ms_step = max_over_ranks(ms_step)
+    value = world * NRHS / (ms_step * 1e-3)
+
+    # ---- e2e: host buffers through tm_tsm_batch_host, H2D + D2H inside the timed region ----
+    for i in range(max(1, args.warmup // 2)):
+        step_e2e(i)
+    barrier()
+    ms_e2e = max_over_ranks(time_events(torch, step_e2e, args.steps))
+    e2e = {"value": world * NRHS / (ms_e2e * 1e-3), "unit": "solves/s", "h2d_bytes_per_step": int(codes_host[0].numel()),
+           "d2h_bytes_per_step": int(loops_host.numel() * 8), "ms_per_step": ms_e2e}
+
+    # ---- roofline of the dominant kernel: the 12-RHS fp16 dslash launches inside the timed steps ----
+    # launches per solve batch: 3 (prepare) + 4 per CG iteration while any rhs is active + 1 (reconstruct) + 4 (true residual);
+    # rhs r is active in iterations 1..iters[r]; bytes follow the active right-hand sides exactly.
+    sp = 24 * prec + 4
+    tot_bytes = tot_flops = 0.0
+    for it in iters_log:
+        tot_bytes += 8 * dslash_bytes(Vh, prec, recon, False, NRHS) + 5 * Vh * NRHS * sp  # 8 full launches, 5 of them read x
+        tot_flops += Vh * NRHS * (3 * FLOPS_XPAY + 1 * FLOPS_TWIST_INV + 2 * (FLOPS_TWIST_INV + FLOPS_XPAY))
+        for k in range(1, max(it) + 1):
+            act = sum(1 for x in it if x >= k)
+            tot_bytes += 4 * Vh * 8 * recon * prec + Vh * act * (4 * 2 + 2) * sp
+            tot_flops += Vh * act * 2 * (FLOPS_TWIST_INV + FLOPS_XPAY)
+    k_avg_ms = k_ms / max(1, k_n)
+    ach_gbs = tot_bytes / (k_ms * 1e-3) / 1e9
+    ach_tf = tot_flops / (k_ms * 1e-3) / 1e12
+    roofline = {"kernel": "dslash_kernel<fp16,recon12,NR=3> x 12 RHS", "bound": "alu", "achieved": ach_tf, "peak": FP32_PEAK_TFLOPS,
+                "unit": "TFLOP/s", "frac": ach_tf / FP32_PEAK_TFLOPS, "traffic": None,
+                "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks)",
+                "avg_launch_ms": k_avg_ms, "launches_timed": int(k_n), "share_of_step": k_ms / (ms_step * args.steps),
+                "hbm_view": {"achieved_GBps": ach_gbs, "peak_GBps": hbm_peak, "frac": ach_gbs / hbm_peak, "peak_source": peak_src}}
+
+    out = {"metric": "LP solves/s", "value": value, "unit": "solves/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f32 (fp16 storage + per-site fp32 norm, fp64 reductions)", "data": "synthetic",
+           "config": {"workload": "32^3x64 TSM (BASELINE.json configs[3]): 12 Z2xiZ2 sources per step, truncated CG tol 1e-2, "
+                                  "12-real links, 12 RHS per gauge load, + 16-Gamma per-timeslice loop of each solution",
+                      "lattice": list(DIMS), "kappa": kappa, "mu": mu, "gauge": "seeded SU(3), eps=0.5", "nrhs": NRHS,
+                      "iters_per_solve": float(np.mean(iters_log)), "l2": "inputs larger than L2 (gauge 201 MB + 12x2x54.5 MB vectors)",
+                      "parallelism": "independent noise batches per GPU (no collective)"},
+           "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
+    if rank == 0:
+        extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world)
+        print(json.dumps(out))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
+    """Rank 0, N=1 context numbers: single-RHS dslash table (BASELINE.json configs[2]), MdagM, mixed CG to 1e-8, loop
+    contraction, and the oracle timed on the host cores."""
+    Vh = L.V // 2
+    kappa, mu = ti.KAPPA, ti.MU
+    psi = torch.from_numpy(ti.z4(DIMS, seed=777).view(np.float64)).cuda()
+    table = {}
+    for prec in (4, 2):
+        pb = tm.tm_spinor_bytes(L, prec, 0, 1)
+        src = tm.device_buffer(2 * pb)
+        tm.tm_spinor_pack(L, psi, prec, 1, src)
+        # rotate through 4 output/x buffers so the spinor working set (>= 5 x 54..101 MB) exceeds the 126 MB L2
+        bufs = [tm.device_buffer(pb) for _ in range(4)]
+        xs = [tm.device_buffer(pb) for _ in range(4)]
+        for b in bufs + xs:
+            b.copy_(src[:pb])
+        tmp = tm.device_buffer(2 * pb)
+        for recon in (18, 12):
+            g = gauges[(prec, recon)]
+            for kind, name, fl in ((tm.TM_KIND_TWIST_INV, "twist_inv", FLOPS_TWIST_INV), (tm.TM_KIND_XPAY_TWIST, "xpay_twist", FLOPS_XPAY)):
+                def run(i, kind=kind, g=g, prec=prec, recon=recon):
+                    tm.tm_dslash(L, g, prec, recon, bufs[i % 4], src[pb:2 * pb], xs[i % 4] if kind == tm.TM_KIND_XPAY_TWIST else None, 0, 0,
+                                 kind, kappa, mu)
+                for i in range(5):
+                    run(i)
+                ms = min(time_events(torch, run, 40) for _ in range(3))
+                by = dslash_bytes(Vh, prec, recon, kind == tm.TM_KIND_XPAY_TWIST)
+                sp = 24 * prec + (4 if prec == 2 else 0)
+                naive = Vh * (8 * recon * prec + (9 + (1 if kind == tm.TM_KIND_XPAY_TWIST else 0)) * sp)
+                gbs = by / ms / 1e6
+                table["%s_fp%d_recon%d" % (name, prec * 8, recon)] = {
+                    "us": ms * 1e3, "GFLOPS": Vh * fl / ms / 1e6, "GBps_algorithmic": gbs, "GBps_naive_model": naive / ms / 1e6,
+                    "bytes_per_site_minimal": by / Vh, "bytes_per_site_naive": naive / Vh,
+                    "frac_of_measured_%.0f" % hbm_peak: gbs / hbm_peak, "frac_of_nominal_8000": gbs / 8000.0}
+            def run_mdagm(i, g=gauges[(prec, 12)], prec=prec):
+                tm.tm_MdagM(L, g, prec, 12, bufs[i % 4], src[:pb], tmp, 0, kappa, mu)
+            for i in range(3):
+                run_mdagm(i)
+            ms = min(time_events(torch, run_mdagm, 20) for _ in range(3))
+            table["MdagM_fp%d_recon12" % (prec * 8)] = {"us": ms * 1e3, "GFLOPS": Vh * 2 * (FLOPS_TWIST_INV + FLOPS_XPAY) / ms / 1e6,
+                                                       "GBps_algorithmic": (2 * dslash_bytes(Vh, prec, 12, False) + 2 * dslash_bytes(Vh, prec, 12, True)) / ms / 1e6}
+        del bufs, xs, src, tmp
+    out["dslash"] = table
+    out["dslash_peak_source"] = peak_src
+
+    # loop contraction alone (fp16, 12 RHS): reads 2 full spinors per rhs
+    prec = 2
+    fb = tm.tm_spinor_bytes(L, prec, 1, NRHS)
+    a, b = tm.device_buffer(fb), tm.device_buffer(fb)
+    a.zero_(); b.zero_()
+    lo = torch.zeros((NRHS, 16, DIMS[3], 2), dtype=torch.float64, device="cuda")
+    lws = tm.device_buffer(tm.tm_loop_workspace_bytes(L, NRHS))
+    f = lambda i: tm.tm_loop_contract(L, a, b, prec, NRHS, lo, lws)
+    f(0)
+    ms = time_events(torch, f, 10)
+    out["loop_contract_fp16_x12"] = {"us": ms * 1e3, "GBps_algorithmic": 2 * fb / ms / 1e6, "frac_of_measured": 2 * fb / ms / 1e6 / hbm_peak}
+    del a, b
+
+    # mixed-precision CG to 1e-8 on one Z2xiZ2 source (configs[2]): fp64 reliable updates, fp32 and fp16 iterations
+    cg = {}
+    pb8 = tm.tm_spinor_bytes(L, 8, 1, 1)
+    eta8, s8 = tm.device_buffer(pb8), tm.device_buffer(pb8)
+    tm.tm_spinor_pack(L, psi, 8, 1, eta8)
+    for plp in (4, 2):
+        ws = tm.device_buffer(tm.tm_cg_workspace_bytes(L, 8, plp, tm.TM_CG_HP_MIXED, 1))
+        prm = tm.make_cg_params(kappa, mu, 1e-8, 5000, tm.TM_CG_HP_MIXED, 0.1, 1)
+        torch.cuda.synchronize()
+        t0 = time.time()
+        rc, info = tm.tm_cg(L, gauges[(8, 12)], 8, gauges[(plp, 12)], plp, 12, s8, eta8, prm, ws)
+        torch.cuda.synchronize()
+        dt = time.time() - t0
+        cg["fp64+fp%d" % (plp * 8)] = {"status": rc, "iters": info.iters, "reliable_updates": info.reliable_updates,
+                                       "true_resid": info.true_resid, "seconds": dt, "ms_per_iter": 1e3 * dt / max(1, info.iters)}
+        del ws
+    out["cg_mixed_1e-8"] = cg
+    if world == 1:
+        base, _ = cpu_oracle_sample()
+        out["cpu_baseline"] = base
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if args.warmup < 3:
+        args.warmup = 3
+    run_b200(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()
