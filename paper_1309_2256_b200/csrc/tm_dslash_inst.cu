@@ -1,5 +1,6 @@
 // tm_dslash_inst.cu -- one translation unit per (TM_PREC, TM_RECON), compiled with -DTM_PREC=.. -DTM_RECON=..
-#include "tm_dslash.cuh"
+#include "tm_dslash_tile.cuh"
+#include <cstdlib>
 
 #ifndef TM_PREC
 #error "compile with -DTM_PREC={8,4,2} -DTM_RECON={18,12}"
@@ -31,10 +32,45 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     if (n % 2 == 0) launch_nr<TM_PREC, TM_RECON, 2>(a, n / 2, st);
     else launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
 #else
-    if (n % 3 == 0) launch_nr<TM_PREC, TM_RECON, 3>(a, n / 3, st);
-    else if (n % 4 == 0) launch_nr<TM_PREC, TM_RECON, 4>(a, n / 4, st);
-    else if (n % 2 == 0) launch_nr<TM_PREC, TM_RECON, 2>(a, n / 2, st);
-    else launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
+    static const int cfg_multi = getenv("TM_DSLASH_MULTI") ? atoi(getenv("TM_DSLASH_MULTI")) : 3;
+    static const int cfg_single = getenv("TM_DSLASH_SINGLE") ? atoi(getenv("TM_DSLASH_SINGLE")) : 0;
+    const bool dg = p.dagger != 0;
+    if (n == 1) {
+        switch (cfg_single) {
+        case 0: launch_tile<TM_PREC, TM_RECON, 128, 1, 4, false, true>(a, dg, st); break;
+        case 1: launch_tile<TM_PREC, TM_RECON, 128, 1, 4, false, false>(a, dg, st); break;
+        case 2: launch_tile<TM_PREC, TM_RECON, 128, 1, 5, false, true>(a, dg, st); break;
+        case 3: launch_tile<TM_PREC, TM_RECON, 64, 1, 8, false, true>(a, dg, st); break;
+        case 4: launch_tile<TM_PREC, TM_RECON, 128, 1, 3, false, true>(a, dg, st); break;
+        case 5: launch_tile<TM_PREC, TM_RECON, 128, 1, 5, false, false>(a, dg, st); break;
+        case 6: launch_tile<TM_PREC, TM_RECON, 128, 1, 6, false, false>(a, dg, st); break;
+        case 7: launch_tile<TM_PREC, TM_RECON, 64, 1, 10, false, false>(a, dg, st); break;
+        case 8: launch_tile<TM_PREC, TM_RECON, 256, 1, 3, false, false>(a, dg, st); break;
+        default: launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
+        }
+    } else {
+        switch (cfg_multi) {
+        case 0: launch_tile<TM_PREC, TM_RECON, 32, 12, 1, true, true>(a, dg, st); break;
+        case 1: launch_tile<TM_PREC, TM_RECON, 32, 12, 2, true, true>(a, dg, st); break;
+        case 2: launch_tile<TM_PREC, TM_RECON, 32, 6, 2, true, true>(a, dg, st); break;
+        case 3: launch_tile<TM_PREC, TM_RECON, 32, 6, 3, true, true>(a, dg, st); break;
+        case 4: launch_tile<TM_PREC, TM_RECON, 32, 4, 4, true, true>(a, dg, st); break;
+        case 5: launch_tile<TM_PREC, TM_RECON, 32, 4, 5, true, true>(a, dg, st); break;
+        case 6: launch_tile<TM_PREC, TM_RECON, 32, 6, 3, true, false>(a, dg, st); break;
+        case 7: launch_tile<TM_PREC, TM_RECON, 32, 4, 4, true, false>(a, dg, st); break;
+        case 8: launch_tile<TM_PREC, TM_RECON, 32, 12, 2, true, false>(a, dg, st); break;
+        case 9: launch_tile<TM_PREC, TM_RECON, 32, 3, 5, true, true>(a, dg, st); break;
+        case 10: launch_tile<TM_PREC, TM_RECON, 32, 6, 4, true, false>(a, dg, st); break;
+        case 11: launch_tile<TM_PREC, TM_RECON, 32, 4, 6, true, false>(a, dg, st); break;
+        case 12: launch_tile<TM_PREC, TM_RECON, 32, 3, 8, true, false>(a, dg, st); break;
+        case 13: launch_tile<TM_PREC, TM_RECON, 32, 2, 12, true, false>(a, dg, st); break;
+        default:
+            if (n % 3 == 0) launch_nr<TM_PREC, TM_RECON, 3>(a, n / 3, st);
+            else if (n % 4 == 0) launch_nr<TM_PREC, TM_RECON, 4>(a, n / 4, st);
+            else if (n % 2 == 0) launch_nr<TM_PREC, TM_RECON, 2>(a, n / 2, st);
+            else launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
+        }
+    }
 #endif
     kernel_timing_end(st);
     TM_LAUNCH_CHECK("dslash_kernel");

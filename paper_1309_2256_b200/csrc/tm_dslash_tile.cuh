@@ -1,0 +1,367 @@
+// tm_dslash_tile.cuh -- fp32 / fp16-storage hopping term, one thread per (site, right-hand side)
+// (SURVEY.md 8(a) rows a2, a3, a7; PAPER.md:384 fused kernels, :403 link reconstruction).
+//
+//   out = (p0 + i p1 g5) x + (q0 + i q1 g5) sum_mu [(1-g_mu) s U_mu(x) in(x+mu) + (1+g_mu) s U_mu(x-mu)^dag in(x-mu)]
+//
+// CTA = S consecutive checkerboard sites (threadIdx.x) x RB right-hand sides (threadIdx.y); a warp is 32 sites
+// of ONE right-hand side, so every spinor access is a fully coalesced 128-bit load.
+//   phase A (SL = links through shared memory, used when nrhs > 1): the CTA's 8*S links are loaded once,
+//     converted to fp32, rebuilt from 12 reals, daggered for the backward hops, multiplied by the antiperiodic
+//     sign and parked in shared memory; the 8 neighbour indices of every site go there too.  All RB right-hand
+//     sides of the tile reuse them ("reuses each gauge link load", BASELINE.json north_star).
+//   phase B: per direction: raw 16-byte chunks of the neighbour (prefetched one direction ahead) -> spin
+//     projection to a half spinor (12 reals) -> SU(3) multiply -> reconstruction into the accumulator.
+// fp16 storage: the projection adds the binary16 words directly in fp32 (FHADD: f32 = f16 + f32, exact
+// inputs), and the per-site norm multiplies the 12 projected-and-rotated reals inside the reconstruction FMAs
+// instead of the 24 loaded ones.  The dagger is a template parameter: all signs are instruction modifiers.
+#pragma once
+#include "tm_dslash.cuh"
+
+namespace tmk {
+
+// ---- raw (unconverted) site data --------------------------------------------------------------------
+template <int PREC> struct Raw;
+template <> struct Raw<4> {
+    float4 q[6];
+};
+template <> struct Raw<2> {
+    uint4 q[3];
+    float nrm;
+};
+
+template <int PREC>
+__device__ __forceinline__ void load_raw(const void* base, int Vh, int cb, Raw<PREC>& r)
+{
+    if constexpr (PREC == 4) {
+        const float4* p = reinterpret_cast<const float4*>(base) + cb;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) r.q[k] = __ldg(p + (size_t)k * Vh);
+    } else {
+        const uint4* p = reinterpret_cast<const uint4*>(base) + cb;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) r.q[k] = __ldg(p + (size_t)k * Vh);
+        r.nrm = __ldg(reinterpret_cast<const float*>(reinterpret_cast<const uint4*>(base) + (size_t)3 * Vh) + cb);
+    }
+}
+
+// binary16 word (re = low half, im = high half) helpers; FHADD takes the half select and the sign as modifiers
+__device__ __forceinline__ float h_lo(uint32_t w)
+{
+    float r;
+    asm("{.reg .b16 l,h; mov.b32 {l,h}, %1; cvt.f32.f16 %0, l;}" : "=f"(r) : "r"(w));
+    return r;
+}
+__device__ __forceinline__ float h_hi(uint32_t w)
+{
+    float r;
+    asm("{.reg .b16 l,h; mov.b32 {l,h}, %1; cvt.f32.f16 %0, h;}" : "=f"(r) : "r"(w));
+    return r;
+}
+// c + sign * (half HI ? high : low of w), sign = NEG ? -1 : +1
+template <int HI, int NEG>
+__device__ __forceinline__ float h_add(uint32_t w, float c)
+{
+    float r;
+    if (HI && NEG) asm("{.reg .b16 l,h; mov.b32 {l,h}, %1; neg.f16 h, h; add.rn.f32.f16 %0, h, %2;}" : "=f"(r) : "r"(w), "f"(c));
+    if (HI && !NEG) asm("{.reg .b16 l,h; mov.b32 {l,h}, %1; add.rn.f32.f16 %0, h, %2;}" : "=f"(r) : "r"(w), "f"(c));
+    if (!HI && NEG) asm("{.reg .b16 l,h; mov.b32 {l,h}, %1; neg.f16 l, l; add.rn.f32.f16 %0, l, %2;}" : "=f"(r) : "r"(w), "f"(c));
+    if (!HI && !NEG) asm("{.reg .b16 l,h; mov.b32 {l,h}, %1; add.rn.f32.f16 %0, l, %2;}" : "=f"(r) : "r"(w), "f"(c));
+    return r;
+}
+
+// complex number (spin s, colour c) of a raw site: accessors for both storage types
+template <int PREC>
+struct Cx {
+    // fp32: value pair; fp16: the packed word
+    float re, im;
+    uint32_t w;
+};
+template <int PREC>
+__device__ __forceinline__ Cx<PREC> raw_cx(const Raw<PREC>& r, int j) // j = s*3 + c, compile-time after unrolling
+{
+    Cx<PREC> z;
+    if constexpr (PREC == 4) {
+        const float4 q = r.q[j >> 1];
+        z.re = (j & 1) ? q.z : q.x;
+        z.im = (j & 1) ? q.w : q.y;
+        z.w = 0;
+    } else {
+        const uint4 q = r.q[j >> 2];
+        z.w = (j & 3) == 0 ? q.x : (j & 3) == 1 ? q.y : (j & 3) == 2 ? q.z : q.w;
+        z.re = z.im = 0;
+    }
+    return z;
+}
+// h = a + SG * b
+template <int PREC, int SG>
+__device__ __forceinline__ void cx_add(const Cx<PREC>& a, const Cx<PREC>& b, float& hr, float& hi)
+{
+    if constexpr (PREC == 4) {
+        hr = SG > 0 ? a.re + b.re : a.re - b.re;
+        hi = SG > 0 ? a.im + b.im : a.im - b.im;
+    } else {
+        hr = h_add<0, (SG < 0)>(b.w, h_lo(a.w));
+        hi = h_add<1, (SG < 0)>(b.w, h_hi(a.w));
+    }
+}
+// h = a + SG * i * b  : hr = ar - SG bi ; hi = ai + SG br
+template <int PREC, int SG>
+__device__ __forceinline__ void cx_addi(const Cx<PREC>& a, const Cx<PREC>& b, float& hr, float& hi)
+{
+    if constexpr (PREC == 4) {
+        hr = SG > 0 ? a.re - b.im : a.re + b.im;
+        hi = SG > 0 ? a.im + b.re : a.im - b.re;
+    } else {
+        hr = h_add<1, (SG > 0)>(b.w, h_lo(a.w));
+        hi = h_add<0, (SG < 0)>(b.w, h_hi(a.w));
+    }
+}
+
+// h[12] = upper half of (1 - E g_mu) psi (un-normalised for fp16: the site norm is applied in tile_reconstruct)
+template <int PREC, int MU, int E>
+__device__ __forceinline__ void tile_project(const Raw<PREC>& r, float* h)
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const Cx<PREC> p0 = raw_cx<PREC>(r, c), p1 = raw_cx<PREC>(r, 3 + c), p2 = raw_cx<PREC>(r, 6 + c), p3 = raw_cx<PREC>(r, 9 + c);
+        if (MU == 0) { // h0 = p0 + E i p3 ; h1 = p1 + E i p2
+            cx_addi<PREC, E>(p0, p3, h[2 * c], h[2 * c + 1]);
+            cx_addi<PREC, E>(p1, p2, h[6 + 2 * c], h[6 + 2 * c + 1]);
+        } else if (MU == 1) { // h0 = p0 + E p3 ; h1 = p1 - E p2
+            cx_add<PREC, E>(p0, p3, h[2 * c], h[2 * c + 1]);
+            cx_add<PREC, -E>(p1, p2, h[6 + 2 * c], h[6 + 2 * c + 1]);
+        } else if (MU == 2) { // h0 = p0 + E i p2 ; h1 = p1 - E i p3
+            cx_addi<PREC, E>(p0, p2, h[2 * c], h[2 * c + 1]);
+            cx_addi<PREC, -E>(p1, p3, h[6 + 2 * c], h[6 + 2 * c + 1]);
+        } else { // h0 = p0 - E p2 ; h1 = p1 - E p3
+            cx_add<PREC, -E>(p0, p2, h[2 * c], h[2 * c + 1]);
+            cx_add<PREC, -E>(p1, p3, h[6 + 2 * c], h[6 + 2 * c + 1]);
+        }
+    }
+}
+
+// acc += w * (g, lower(g)), lower rebuilt from the upper half; w = site norm (fp16) or absent (fp32)
+template <int MU, int E, bool SCALED>
+__device__ __forceinline__ void tile_reconstruct(float* acc, const float* g, float w)
+{
+    const float wp = SCALED ? w : 1.f;
+    const float we = (E > 0) ? wp : -wp; // E * w
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float g0r = g[2 * c], g0i = g[2 * c + 1], g1r = g[6 + 2 * c], g1i = g[6 + 2 * c + 1];
+        acc[2 * c] = fmaf(wp, g0r, acc[2 * c]);
+        acc[2 * c + 1] = fmaf(wp, g0i, acc[2 * c + 1]);
+        acc[6 + 2 * c] = fmaf(wp, g1r, acc[6 + 2 * c]);
+        acc[6 + 2 * c + 1] = fmaf(wp, g1i, acc[6 + 2 * c + 1]);
+        if (MU == 0) { // lower = (-E i g1, -E i g0)
+            acc[12 + 2 * c] = fmaf(we, g1i, acc[12 + 2 * c]);
+            acc[12 + 2 * c + 1] = fmaf(-we, g1r, acc[12 + 2 * c + 1]);
+            acc[18 + 2 * c] = fmaf(we, g0i, acc[18 + 2 * c]);
+            acc[18 + 2 * c + 1] = fmaf(-we, g0r, acc[18 + 2 * c + 1]);
+        } else if (MU == 1) { // lower = (-E g1, E g0)
+            acc[12 + 2 * c] = fmaf(-we, g1r, acc[12 + 2 * c]);
+            acc[12 + 2 * c + 1] = fmaf(-we, g1i, acc[12 + 2 * c + 1]);
+            acc[18 + 2 * c] = fmaf(we, g0r, acc[18 + 2 * c]);
+            acc[18 + 2 * c + 1] = fmaf(we, g0i, acc[18 + 2 * c + 1]);
+        } else if (MU == 2) { // lower = (-E i g0, E i g1)
+            acc[12 + 2 * c] = fmaf(we, g0i, acc[12 + 2 * c]);
+            acc[12 + 2 * c + 1] = fmaf(-we, g0r, acc[12 + 2 * c + 1]);
+            acc[18 + 2 * c] = fmaf(-we, g1i, acc[18 + 2 * c]);
+            acc[18 + 2 * c + 1] = fmaf(we, g1r, acc[18 + 2 * c + 1]);
+        } else { // lower = (-E g0, -E g1)
+            acc[12 + 2 * c] = fmaf(-we, g0r, acc[12 + 2 * c]);
+            acc[12 + 2 * c + 1] = fmaf(-we, g0i, acc[12 + 2 * c + 1]);
+            acc[18 + 2 * c] = fmaf(-we, g1r, acc[18 + 2 * c]);
+            acc[18 + 2 * c + 1] = fmaf(-we, g1i, acc[18 + 2 * c + 1]);
+        }
+    }
+}
+
+// neighbour indices of checkerboard site cb (order: +x -x +y -y +z -z +t -t) and the two temporal hop signs
+__device__ __forceinline__ void tile_neighbours(const Geo& g, int parity, int cb, int* nb, float& sgp, float& sgm)
+{
+    uint32_t t, rem, z, rem2, y, xh;
+    g.dXh.divmod((uint32_t)cb, rem, xh);
+    g.dY.divmod(rem, rem2, y);
+    g.dZ.divmod(rem2, t, z);
+    const int xodd = (parity + y + z + t) & 1;
+    const int Xh = g.Xh, XhY = g.XhY, V3h = g.V3h, Vh = g.Vh;
+    nb[0] = cb + (xodd ? ((int)xh == Xh - 1 ? 1 - Xh : 1) : 0);
+    nb[1] = cb - (xodd ? 0 : ((int)xh == 0 ? 1 - Xh : 1));
+    nb[2] = cb + ((int)y == g.Y - 1 ? Xh - XhY : Xh);
+    nb[3] = cb - ((int)y == 0 ? Xh - XhY : Xh);
+    nb[4] = cb + ((int)z == g.Z - 1 ? XhY - V3h : XhY);
+    nb[5] = cb - ((int)z == 0 ? XhY - V3h : XhY);
+    nb[6] = cb + ((int)t == g.T - 1 ? V3h - Vh : V3h);
+    nb[7] = cb - ((int)t == 0 ? V3h - Vh : V3h);
+    sgp = (g.ap && (int)t == g.T - 1) ? -1.f : 1.f;
+    sgm = (g.ap && (int)t == 0) ? -1.f : 1.f;
+}
+
+template <int S>
+struct TileSmem {
+    int nbr[8][S];
+    float4 u4[8][4][S];
+    float2 u2[8][S];
+};
+
+template <int PREC, int RECON, int DAG, int S, int RB, int MINB, bool SL, bool PF>
+__global__ void __launch_bounds__(S* RB, MINB) dslash_tile_kernel(const DslashKArgs a)
+{
+    constexpr int E = DAG ? -1 : 1;
+    constexpr bool SC = (PREC == 2);
+    __shared__ TileSmem<SL ? S : 1> sm;
+
+    const int tx = threadIdx.x, ty = threadIdx.y;
+    const int ny = (a.nrhs + RB - 1) / RB;
+    const int tile = blockIdx.x / ny, by = blockIdx.x - tile * ny; // rhs groups of one tile are adjacent in launch order
+    const int cb0 = tile * S, cb = cb0 + tx, Vh = a.g.Vh;
+    const int rhs = by * RB + ty;
+    const bool valid = cb < Vh;
+    const bool act = valid && rhs < a.nrhs && (a.active == nullptr || a.active[rhs] != 0);
+
+    int nb[8];
+    if constexpr (SL) {
+        if (__syncthreads_or(act) == 0) return;
+        if (ty == 0 && valid) {
+            float sgp, sgm;
+            tile_neighbours(a.g, a.parity, cb, nb, sgp, sgm);
+#pragma unroll
+            for (int d = 0; d < 8; ++d) sm.nbr[d][tx] = (d == 6 && sgp < 0.f) || (d == 7 && sgm < 0.f) ? ~nb[d] : nb[d];
+        }
+        __syncthreads();
+        // phase A: links of the tile -> fp32, rebuilt, daggered for backward hops, signed, in shared memory
+        for (int l = ty * S + tx; l < 8 * S; l += S * RB) {
+            const int d = l / S, s = l - d * S;
+            if (cb0 + s >= Vh) continue;
+            const bool fwd = !(d & 1);
+            int nbi = sm.nbr[d][s];
+            const float sg = nbi < 0 ? -1.f : 1.f;
+            nbi = nbi < 0 ? ~nbi : nbi;
+            const char* blk = a.gauge + (size_t)((fwd ? a.parity : 1 - a.parity) * 4 + (d >> 1)) * a.link_block;
+            float u[18];
+            load_link<PREC, RECON>(blk, Vh, fwd ? cb0 + s : nbi, u);
+            float w[18];
+#pragma unroll
+            for (int i = 0; i < 3; ++i)
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    w[2 * (i * 3 + j)] = sg * (fwd ? u[2 * (i * 3 + j)] : u[2 * (j * 3 + i)]);
+                    w[2 * (i * 3 + j) + 1] = sg * (fwd ? u[2 * (i * 3 + j) + 1] : -u[2 * (j * 3 + i) + 1]);
+                }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) sm.u4[d][k][s] = make_float4(w[4 * k], w[4 * k + 1], w[4 * k + 2], w[4 * k + 3]);
+            sm.u2[d][s] = make_float2(w[16], w[17]);
+        }
+        __syncthreads();
+        if (!act) return;
+#pragma unroll
+        for (int d = 0; d < 8; ++d) {
+            const int v = sm.nbr[d][tx];
+            nb[d] = v < 0 ? ~v : v;
+        }
+    }
+    float sgp = 1.f, sgm = 1.f;
+    if constexpr (!SL) {
+        if (!act) return;
+        tile_neighbours(a.g, a.parity, cb, nb, sgp, sgm);
+    }
+
+    const char* in = a.in + (size_t)rhs * a.stride_in;
+    float acc[24];
+#pragma unroll
+    for (int k = 0; k < 24; ++k) acc[k] = 0.f;
+
+    Raw<PREC> cur, nxt;
+    if constexpr (PF) load_raw<PREC>(in, Vh, nb[0], nxt);
+
+#pragma unroll
+    for (int d = 0; d < 8; ++d) {
+        if constexpr (PF) {
+            cur = nxt;
+            if (d < 7) load_raw<PREC>(in, Vh, nb[d + 1 < 8 ? d + 1 : 7], nxt);
+        } else {
+            load_raw<PREC>(in, Vh, nb[d], cur);
+        }
+        float u[18];
+        if constexpr (SL) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const float4 q = sm.u4[d][k][tx];
+                u[4 * k] = q.x;
+                u[4 * k + 1] = q.y;
+                u[4 * k + 2] = q.z;
+                u[4 * k + 3] = q.w;
+            }
+            const float2 q2 = sm.u2[d][tx];
+            u[16] = q2.x;
+            u[17] = q2.y;
+        } else {
+            const bool fwd = !(d & 1);
+            const char* blk = a.gauge + (size_t)((fwd ? a.parity : 1 - a.parity) * 4 + (d >> 1)) * a.link_block;
+            load_link<PREC, RECON>(blk, Vh, fwd ? cb : nb[d], u);
+        }
+        float h[12], g[12];
+        float w = 1.f;
+        if constexpr (SC) w = cur.nrm;
+        // direction d = 2*mu + (backward): projector sign E for forward, -E for backward
+        if (d == 0) tile_project<PREC, 0, E>(cur, h);
+        if (d == 1) tile_project<PREC, 0, -E>(cur, h);
+        if (d == 2) tile_project<PREC, 1, E>(cur, h);
+        if (d == 3) tile_project<PREC, 1, -E>(cur, h);
+        if (d == 4) tile_project<PREC, 2, E>(cur, h);
+        if (d == 5) tile_project<PREC, 2, -E>(cur, h);
+        if (d == 6) tile_project<PREC, 3, E>(cur, h);
+        if (d == 7) tile_project<PREC, 3, -E>(cur, h);
+        if constexpr (SL) {
+            su3_mul<0>(u, h, g);
+        } else {
+            if (d & 1) su3_mul<1>(u, h, g);
+            else su3_mul<0>(u, h, g);
+            if (d == 6) w *= sgp;
+            if (d == 7) w *= sgm;
+        }
+        if (d == 0) tile_reconstruct<0, E, true>(acc, g, w);
+        if (d == 1) tile_reconstruct<0, -E, true>(acc, g, w);
+        if (d == 2) tile_reconstruct<1, E, true>(acc, g, w);
+        if (d == 3) tile_reconstruct<1, -E, true>(acc, g, w);
+        if (d == 4) tile_reconstruct<2, E, true>(acc, g, w);
+        if (d == 5) tile_reconstruct<2, -E, true>(acc, g, w);
+        if (d == 6) tile_reconstruct<3, E, true>(acc, g, w);
+        if (d == 7) tile_reconstruct<3, -E, true>(acc, g, w);
+    }
+
+    // epilogue: out = (p0 + i p1 g5) x + (q0 + i q1 g5) acc ; g5 = diag(1,1,-1,-1)
+    const float p0 = (float)a.pq[0], p1 = (float)a.pq[1], q0 = (float)a.pq[2], q1 = (float)a.pq[3];
+    float o[24];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+        const float s5 = (k < 6) ? 1.f : -1.f;
+        const float dr = acc[2 * k], di = acc[2 * k + 1];
+        o[2 * k] = q0 * dr - s5 * q1 * di;
+        o[2 * k + 1] = q0 * di + s5 * q1 * dr;
+    }
+    if (a.x != nullptr) {
+        float xv[24];
+        load_spinor<PREC>(a.x + (size_t)rhs * a.stride_x, Vh, cb, xv);
+#pragma unroll
+        for (int k = 0; k < 12; ++k) {
+            const float s5 = (k < 6) ? 1.f : -1.f;
+            o[2 * k] += p0 * xv[2 * k] - s5 * p1 * xv[2 * k + 1];
+            o[2 * k + 1] += p0 * xv[2 * k + 1] + s5 * p1 * xv[2 * k];
+        }
+    }
+    store_spinor<PREC>(a.out + (size_t)rhs * a.stride_out, Vh, cb, o);
+}
+
+template <int PREC, int RECON, int S, int RB, int MINB, bool SL, bool PF>
+static inline void launch_tile(const DslashKArgs& a, bool dagger, cudaStream_t st)
+{
+    const int ny = (a.nrhs + RB - 1) / RB;
+    const unsigned tiles = (unsigned)((a.g.Vh + S - 1) / S);
+    dim3 block(S, RB), grid(tiles * ny);
+    if (dagger) dslash_tile_kernel<PREC, RECON, 1, S, RB, MINB, SL, PF><<<grid, block, 0, st>>>(a);
+    else dslash_tile_kernel<PREC, RECON, 0, S, RB, MINB, SL, PF><<<grid, block, 0, st>>>(a);
+}
+
+} // namespace tmk
