@@ -32,8 +32,8 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     if (n % 2 == 0) launch_nr<TM_PREC, TM_RECON, 2>(a, n / 2, st);
     else launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
 #else
-    static const int cfg_multi = getenv("TM_DSLASH_MULTI") ? atoi(getenv("TM_DSLASH_MULTI")) : 3;
-    static const int cfg_single = getenv("TM_DSLASH_SINGLE") ? atoi(getenv("TM_DSLASH_SINGLE")) : 0;
+    static const int cfg_multi = getenv("TM_DSLASH_MULTI") ? atoi(getenv("TM_DSLASH_MULTI")) : 8;
+    static const int cfg_single = getenv("TM_DSLASH_SINGLE") ? atoi(getenv("TM_DSLASH_SINGLE")) : (TM_PREC == 2 ? 2 : 1);
     const bool dg = p.dagger != 0;
     if (n == 1) {
         switch (cfg_single) {
