@@ -32,7 +32,10 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     if (n % 2 == 0) launch_nr<TM_PREC, TM_RECON, 2>(a, n / 2, st);
     else launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
 #else
-    static const int cfg_multi = getenv("TM_DSLASH_MULTI") ? atoi(getenv("TM_DSLASH_MULTI")) : 8;
+    // Launch shapes from the B200 sweep; the environment knobs exist for re-tuning:
+    //   TM_DSLASH_SINGLE: 0 = 128 registers + prefetch, 1 = 128 registers, 2 = 96 registers + prefetch, -1 = dslash_kernel
+    //   TM_DSLASH_MULTI : 0 = by nrhs (12 / 6 / 4 right-hand sides per CTA at 80 registers), 1 = 12 + prefetch, -1 = dslash_kernel
+    static const int cfg_multi = getenv("TM_DSLASH_MULTI") ? atoi(getenv("TM_DSLASH_MULTI")) : 0;
     static const int cfg_single = getenv("TM_DSLASH_SINGLE") ? atoi(getenv("TM_DSLASH_SINGLE")) : (TM_PREC == 2 ? 2 : 1);
     const bool dg = p.dagger != 0;
     if (n == 1) {
@@ -40,36 +43,19 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
         case 0: launch_tile<TM_PREC, TM_RECON, 128, 1, 4, false, true>(a, dg, st); break;
         case 1: launch_tile<TM_PREC, TM_RECON, 128, 1, 4, false, false>(a, dg, st); break;
         case 2: launch_tile<TM_PREC, TM_RECON, 128, 1, 5, false, true>(a, dg, st); break;
-        case 3: launch_tile<TM_PREC, TM_RECON, 64, 1, 8, false, true>(a, dg, st); break;
-        case 4: launch_tile<TM_PREC, TM_RECON, 128, 1, 3, false, true>(a, dg, st); break;
-        case 5: launch_tile<TM_PREC, TM_RECON, 128, 1, 5, false, false>(a, dg, st); break;
-        case 6: launch_tile<TM_PREC, TM_RECON, 128, 1, 6, false, false>(a, dg, st); break;
-        case 7: launch_tile<TM_PREC, TM_RECON, 64, 1, 10, false, false>(a, dg, st); break;
-        case 8: launch_tile<TM_PREC, TM_RECON, 256, 1, 3, false, false>(a, dg, st); break;
         default: launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
         }
+    } else if (cfg_multi == 0) {
+        if (n <= 4) launch_tile<TM_PREC, TM_RECON, 32, 4, 6, true, false>(a, dg, st);
+        else if (n <= 6) launch_tile<TM_PREC, TM_RECON, 32, 6, 4, true, false>(a, dg, st);
+        else launch_tile<TM_PREC, TM_RECON, 32, 12, 2, true, false>(a, dg, st);
+    } else if (cfg_multi == 1) {
+        launch_tile<TM_PREC, TM_RECON, 32, 12, 2, true, true>(a, dg, st);
     } else {
-        switch (cfg_multi) {
-        case 0: launch_tile<TM_PREC, TM_RECON, 32, 12, 1, true, true>(a, dg, st); break;
-        case 1: launch_tile<TM_PREC, TM_RECON, 32, 12, 2, true, true>(a, dg, st); break;
-        case 2: launch_tile<TM_PREC, TM_RECON, 32, 6, 2, true, true>(a, dg, st); break;
-        case 3: launch_tile<TM_PREC, TM_RECON, 32, 6, 3, true, true>(a, dg, st); break;
-        case 4: launch_tile<TM_PREC, TM_RECON, 32, 4, 4, true, true>(a, dg, st); break;
-        case 5: launch_tile<TM_PREC, TM_RECON, 32, 4, 5, true, true>(a, dg, st); break;
-        case 6: launch_tile<TM_PREC, TM_RECON, 32, 6, 3, true, false>(a, dg, st); break;
-        case 7: launch_tile<TM_PREC, TM_RECON, 32, 4, 4, true, false>(a, dg, st); break;
-        case 8: launch_tile<TM_PREC, TM_RECON, 32, 12, 2, true, false>(a, dg, st); break;
-        case 9: launch_tile<TM_PREC, TM_RECON, 32, 3, 5, true, true>(a, dg, st); break;
-        case 10: launch_tile<TM_PREC, TM_RECON, 32, 6, 4, true, false>(a, dg, st); break;
-        case 11: launch_tile<TM_PREC, TM_RECON, 32, 4, 6, true, false>(a, dg, st); break;
-        case 12: launch_tile<TM_PREC, TM_RECON, 32, 3, 8, true, false>(a, dg, st); break;
-        case 13: launch_tile<TM_PREC, TM_RECON, 32, 2, 12, true, false>(a, dg, st); break;
-        default:
-            if (n % 3 == 0) launch_nr<TM_PREC, TM_RECON, 3>(a, n / 3, st);
-            else if (n % 4 == 0) launch_nr<TM_PREC, TM_RECON, 4>(a, n / 4, st);
-            else if (n % 2 == 0) launch_nr<TM_PREC, TM_RECON, 2>(a, n / 2, st);
-            else launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
-        }
+        if (n % 3 == 0) launch_nr<TM_PREC, TM_RECON, 3>(a, n / 3, st);
+        else if (n % 4 == 0) launch_nr<TM_PREC, TM_RECON, 4>(a, n / 4, st);
+        else if (n % 2 == 0) launch_nr<TM_PREC, TM_RECON, 2>(a, n / 2, st);
+        else launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
     }
 #endif
     kernel_timing_end(st);
