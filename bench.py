@@ -170,7 +170,7 @@ def run_b200(args, rank, world, local_rank):
     loops = torch.zeros((NRHS, 16, T, 2), dtype=torch.float64, device="cuda")
     tsm_ws = tm.device_buffer(tm.tm_tsm_workspace_bytes(L, prec, NRHS))
     loops_host = torch.zeros((NRHS, 16, T, 2), dtype=torch.float64).pin_memory()
-    prm = tm.make_cg_params(kappa, mu, LP_TOL, 500, tm.TM_CG_LP_TRUNCATED, 0.1, 4)
+    prm = tm.make_cg_params(kappa, mu, LP_TOL, 500, tm.TM_CG_LP_TRUNCATED, 0.1, 4, 1)  # truncated mode: no residual recomputation
     iters_log = []
 
     def step(i):
@@ -225,13 +225,13 @@ def run_b200(args, rank, world, local_rank):
            "d2h_bytes_per_step": int(loops_host.numel() * 8), "ms_per_step": ms_e2e}
 
     # ---- roofline of the dominant kernel: the 12-RHS fp16 dslash launches inside the timed steps ----
-    # launches per solve batch: 3 (prepare) + 4 per CG iteration while any rhs is active + 1 (reconstruct) + 4 (true residual);
+    # launches per solve batch: 3 (prepare) + 4 per CG iteration while any rhs is active + 1 (reconstruct);
     # rhs r is active in iterations 1..iters[r]; bytes follow the active right-hand sides exactly.
     sp = 24 * prec + 4
     tot_bytes = tot_flops = 0.0
     for it in iters_log:
-        tot_bytes += 8 * dslash_bytes(Vh, prec, recon, False, NRHS) + 5 * Vh * NRHS * sp  # 8 full launches, 5 of them read x
-        tot_flops += Vh * NRHS * (3 * FLOPS_XPAY + 1 * FLOPS_TWIST_INV + 2 * (FLOPS_TWIST_INV + FLOPS_XPAY))
+        tot_bytes += 4 * dslash_bytes(Vh, prec, recon, False, NRHS) + 3 * Vh * NRHS * sp  # 4 full launches, 3 of them read x
+        tot_flops += Vh * NRHS * (3 * FLOPS_XPAY + 1 * FLOPS_TWIST_INV)
         for k in range(1, max(it) + 1):
             act = sum(1 for x in it if x >= k)
             tot_bytes += 4 * Vh * 8 * recon * prec + Vh * act * (4 * 2 + 2) * sp
@@ -239,7 +239,7 @@ def run_b200(args, rank, world, local_rank):
     k_avg_ms = k_ms / max(1, k_n)
     ach_gbs = tot_bytes / (k_ms * 1e-3) / 1e9
     ach_tf = tot_flops / (k_ms * 1e-3) / 1e12
-    roofline = {"kernel": "dslash_kernel<fp16,recon12,NR=3> x 12 RHS", "bound": "alu", "achieved": ach_tf, "peak": FP32_PEAK_TFLOPS,
+    roofline = {"kernel": "dslash_tile_kernel<fp16,recon12,32 sites x 12 rhs per CTA>", "bound": "alu", "achieved": ach_tf, "peak": FP32_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": ach_tf / FP32_PEAK_TFLOPS, "traffic": None,
                 "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks)",
                 "avg_launch_ms": k_avg_ms, "launches_timed": int(k_n), "share_of_step": k_ms / (ms_step * args.steps),

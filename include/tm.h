@@ -114,6 +114,8 @@ typedef struct {
     int mode;              /* tm_cg_mode */
     double reliable_delta; /* HP_MIXED: recompute the true residual in prec_hp when |r| drops by this factor (0 -> 0.1) */
     int check_every;       /* host polls the device convergence flag every this many iterations (0 -> 4) */
+    int skip_true_resid;   /* LP_TRUNCATED: 1 = do not recompute |b'' - A x| after the solve (saves one M^dag M);
+                              info.true_resid is then -1.  The truncated mode never uses it. */
 } tm_cg_params;
 
 typedef struct {

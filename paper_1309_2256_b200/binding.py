@@ -26,7 +26,8 @@ ABI_SYMBOLS = [
 
 class tm_cg_params(ctypes.Structure):
     _fields_ = [("kappa", ctypes.c_double), ("mu", ctypes.c_double), ("tol", ctypes.c_double), ("max_iter", ctypes.c_int),
-                ("mode", ctypes.c_int), ("reliable_delta", ctypes.c_double), ("check_every", ctypes.c_int)]
+                ("mode", ctypes.c_int), ("reliable_delta", ctypes.c_double), ("check_every", ctypes.c_int),
+                ("skip_true_resid", ctypes.c_int)]
 
 
 class tm_cg_info(ctypes.Structure):
@@ -197,8 +198,8 @@ def tm_cg_workspace_bytes(L, prec_hp, prec_lp, mode, nrhs=1):
     return load().tm_cg_workspace_bytes(L.handle, prec_hp, prec_lp, mode, nrhs)
 
 
-def make_cg_params(kappa, mu, tol, max_iter, mode, reliable_delta=0.1, check_every=4):
-    return tm_cg_params(kappa, mu, tol, max_iter, mode, reliable_delta, check_every)
+def make_cg_params(kappa, mu, tol, max_iter, mode, reliable_delta=0.1, check_every=4, skip_true_resid=0):
+    return tm_cg_params(kappa, mu, tol, max_iter, mode, reliable_delta, check_every, skip_true_resid)
 
 
 _SOFT = (TM_ERR_MAXITER, TM_ERR_BREAKDOWN)

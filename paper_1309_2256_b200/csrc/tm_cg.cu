@@ -229,8 +229,10 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
     }
     if ((rc = reconstruct_odd(g, gauge, prec, recon, s_full, eta_full, prm->kappa, prm->mu, nrhs, st)) != TM_OK) return rc;
     // recomputed residual of the normal system, in the same storage/arithmetic: Ap = A x; Ap = b - Ap
-    if ((rc = mdagm_apply(g, gauge, prec, recon, Ap, pb, s_full, 2 * pb, t1, 0, prm->kappa, prm->mu, nrhs, nullptr, st)) != TM_OK) return rc;
-    if ((rc = k_axpby<1>(g, prec, prec, V_(Ap, pb), V_(b, pb), -1.0, 1.0, c, nrhs, st)) != TM_OK) return rc;
+    if (!prm->skip_true_resid) {
+        if ((rc = mdagm_apply(g, gauge, prec, recon, Ap, pb, s_full, 2 * pb, t1, 0, prm->kappa, prm->mu, nrhs, nullptr, st)) != TM_OK) return rc;
+        if ((rc = k_axpby<1>(g, prec, prec, V_(Ap, pb), V_(b, pb), -1.0, 1.0, c, nrhs, st)) != TM_OK) return rc;
+    }
     std::vector<CgScal> h(nrhs);
     TM_CUDA_CHECK(cudaMemcpyAsync(h.data(), c.scal, sizeof(CgScal) * nrhs, cudaMemcpyDeviceToHost, st));
     TM_CUDA_CHECK(cudaStreamSynchronize(st));
@@ -240,7 +242,7 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
         info[q].status = h[q].status;
         info[q].reliable_updates = 0;
         info[q].iterated_resid = h[q].b2 > 0 ? std::sqrt(h[q].rr / h[q].b2) : 0.0;
-        info[q].true_resid = h[q].b2 > 0 ? std::sqrt(h[q].aux / h[q].b2) : 0.0;
+        info[q].true_resid = prm->skip_true_resid ? -1.0 : (h[q].b2 > 0 ? std::sqrt(h[q].aux / h[q].b2) : 0.0);
         if (h[q].b2 == 0.0) info[q].status = TM_OK;
         if (info[q].status == TM_ERR_MAXITER && prm->tol == 0.0) info[q].status = TM_OK; // fixed-iteration truncation
         if (info[q].status != TM_OK && (worst == TM_OK || info[q].status == TM_ERR_BREAKDOWN)) worst = info[q].status;

@@ -103,6 +103,27 @@ def test_cg_zero_source_and_mixed_convergence_times():
         assert rel(oracle.M(U, s[r], KAPPA, MU), eta[r]) < 1e-4
 
 
+def test_skip_true_resid_changes_nothing_but_the_report():
+    """tm_cg_params.skip_true_resid drops the diagnostic M^dag M after a truncated solve: same solution bit for bit."""
+    dims = (8, 8, 8, 16)
+    F, U = fields(dims)
+    nrhs, prec, recon = 5, 2, 12  # 5: also covers a right-hand-side count that does not fill the CTA's rhs rows
+    eta = np.stack([ti.z4(dims, seed=800 + r) for r in range(nrhs)])
+    pe = F.pack(eta, prec)
+    ws = tm.device_buffer(tm.tm_cg_workspace_bytes(F.L, 8, prec, tm.TM_CG_LP_TRUNCATED, nrhs))
+    sols = []
+    for skip in (0, 1):
+        s = F.zeros_full(prec, nrhs)
+        prm = tm.make_cg_params(KAPPA, MU, 1e-2, 500, tm.TM_CG_LP_TRUNCATED, 0.1, 4, skip)
+        rc, info = tm.tm_cg_multi(F.L, None, 8, F.gauge(prec, recon), prec, recon, s, pe, prm, nrhs, ws)
+        assert rc == tm.TM_OK
+        for r in range(nrhs):
+            assert info[r].iterated_resid <= 1e-2
+            assert (info[r].true_resid == -1.0) if skip else (0 < info[r].true_resid < 1.3e-2)
+        sols.append(s.clone())
+    assert torch.equal(sols[0], sols[1])
+
+
 def test_tsm_batch_host_end_to_end():
     """H2D of Z2xiZ2 codes -> pack -> batched truncated CG -> 16-Gamma loop per time slice -> D2H, one call."""
     dims = (8, 8, 8, 16)
