@@ -32,6 +32,10 @@ FLOPS_HOP, FLOPS_TWIST_INV, FLOPS_XPAY = 1320, 1392, 1416  # per output site (DE
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12          # 148 SMs x 128 FP32 lanes x 2 (FMA) x max SM clock
 
 
+# one `ncu --set full` capture of the dominant kernel (profiles/r01_ncu_dslash_fp16_recon12_12rhs.md), bytes per launch
+NCU_DRAM_BYTES_PER_LAUNCH = 1.9256e9
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -240,7 +244,8 @@ def run_b200(args, rank, world, local_rank):
     ach_gbs = tot_bytes / (k_ms * 1e-3) / 1e9
     ach_tf = tot_flops / (k_ms * 1e-3) / 1e12
     roofline = {"kernel": "dslash_tile_kernel<fp16,recon12,32 sites x 12 rhs per CTA>", "bound": "alu", "achieved": ach_tf, "peak": FP32_PEAK_TFLOPS,
-                "unit": "TFLOP/s", "frac": ach_tf / FP32_PEAK_TFLOPS, "traffic": None,
+                "unit": "TFLOP/s", "frac": ach_tf / FP32_PEAK_TFLOPS, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
+                "traffic_source": "profiles/r01_ncu_dslash_fp16_recon12_12rhs.md: dram__bytes_read.sum + dram__bytes_write.sum, mean of 4 launches (2 TWIST_INV + 2 XPAY_TWIST, 12 active rhs); algorithmic mean 1.837e9",
                 "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks)",
                 "avg_launch_ms": k_avg_ms, "launches_timed": int(k_n), "share_of_step": k_ms / (ms_step * args.steps),
                 "hbm_view": {"achieved_GBps": ach_gbs, "peak_GBps": hbm_peak, "frac": ach_gbs / hbm_peak, "peak_source": peak_src}}
