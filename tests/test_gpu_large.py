@@ -1,0 +1,120 @@
+"""-m gpu: parity at BASELINE.json's full sizes, in the launch configurations bench.py times.
+
+* 32^3x64 (configs[2], [3]): the 12-right-hand-side fp16 / 12-real tile kernel and the single-rhs kernels, whole fields
+  against the oracle stencil.
+* 64^3x128 (configs[4]): sampled output sites (random + every site of two boundary-touching 2-D planes) against the
+  single-site oracle `hop_gathered`, whose inputs are regenerated from the counter-based generators.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import tm_inputs as ti
+import paper_1309_2256_b200 as tm
+from tm_harness import Fields, TOL, rel, to_dev, gather_site_inputs
+
+pytestmark = pytest.mark.gpu
+KAPPA, MU = ti.KAPPA, ti.MU
+A = 2 * KAPPA * MU
+
+
+def test_32x64_twelve_rhs_dslash_whole_field():
+    """configs[3] launch shape: fp16 storage, 12-real links, 12 right-hand sides per gauge load, both epilogue kinds."""
+    dims = (32, 32, 32, 64)
+    nrhs, prec, recon = 12, 2, 12
+    U = ti.gauge(dims)
+    F = Fields(dims, U, True)
+    codes = np.stack([ti.z4_codes(dims, seed=ti.NOISE_SEED + r) for r in range(nrhs)])
+    pin = tm.device_buffer(tm.tm_spinor_bytes(F.L, prec, 1, nrhs))
+    tm.tm_spinor_pack_z4(F.L, to_dev(codes), prec, nrhs, pin)
+    del codes
+    out = F.zeros_full(prec, nrhs)
+    src_o = F.half(pin, prec, 1, nrhs)
+    x_e = F.half(pin, prec, 0, nrhs)
+    for kind, dagger in ((tm.TM_KIND_TWIST_INV, 0), (tm.TM_KIND_XPAY_TWIST, 1)):
+        res = tm.device_buffer(F.pb(prec) * nrhs)
+        tm.tm_dslash(F.L, F.gauge(prec, recon), prec, recon, res, src_o, x_e if kind == tm.TM_KIND_XPAY_TWIST else None, 0, dagger,
+                     kind, KAPPA, MU, nrhs)
+        out.zero_()
+        F.put_half(out, res, prec, 0, nrhs)
+        got = F.unpack(out, prec, nrhs=nrhs)
+        for r in (0, 5, 11):
+            eta = ti.z4(dims, seed=ti.NOISE_SEED + r)
+            d = oracle.hop(U, oracle.project(eta, 1), ap=True, dagger=bool(dagger))
+            a = -A if dagger else A
+            if kind == tm.TM_KIND_TWIST_INV:
+                ref = oracle.twist(d, a, inverse=True)
+            else:
+                ref = oracle.twist(oracle.project(eta, 0), a) - KAPPA ** 2 * d
+            ref = oracle.project(ref, 0)
+            assert rel(got[r], ref) < TOL[prec], (kind, dagger, r)
+
+
+@pytest.mark.parametrize("prec,recon", [(4, 18), (4, 12), (2, 18), (2, 12)])
+def test_32x64_single_rhs_dslash_whole_field(prec, recon):
+    """configs[2]: the single-rhs kernels bench.py's dslash table times."""
+    dims = (32, 32, 32, 64)
+    U = ti.gauge(dims)
+    F = Fields(dims, U, True)
+    eta = ti.z4(dims, seed=777)
+    pin = F.pack(eta, prec)
+    out = F.zeros_full(prec)
+    tm.tm_dslash(F.L, F.gauge(prec, recon), prec, recon, F.half(out, prec, 1), F.half(pin, prec, 0), None, 1, 0, tm.TM_KIND_TWIST_INV,
+                 KAPPA, MU)
+    ref = oracle.project(oracle.twist(oracle.hop(U, oracle.project(eta, 0), ap=True), A, inverse=True), 1)
+    assert rel(F.unpack(out, prec), ref) < TOL[prec]
+
+
+def _sample_sites(dims, parity, n_random, seed):
+    """Global indices of output sites of `parity`: random ones plus all sites of the planes (x, t) at y = z = 0 and
+    (y, z) at x = X-1, t = T-1, which touch every wrap-around of the lattice."""
+    X, Y, Z, T = dims
+    rng = np.random.default_rng(seed)
+    s = rng.integers(0, X * Y * Z * T, size=2 * n_random)
+    xs, ts = np.meshgrid(np.arange(X), np.arange(T), indexing="ij")
+    ys, zs = np.meshgrid(np.arange(Y), np.arange(Z), indexing="ij")
+    plane1 = ti.site_index(dims, xs.ravel(), 0, 0, ts.ravel())
+    plane2 = ti.site_index(dims, X - 1, ys.ravel(), zs.ravel(), T - 1)
+    s = np.unique(np.concatenate([s, plane1, plane2]))
+    c = (s % X) + ((s // X) % Y) + ((s // (X * Y)) % Z) + (s // (X * Y * Z))
+    return s[(c & 1) == parity]
+
+
+def test_64x128_dslash_sampled_sites():
+    """configs[4]: 33.5 M sites.  TWIST_INV hop, fp32 and fp16 storage, 18- and 12-real links, both output parities,
+    checked on ~6e4 sampled sites per case against the single-site oracle."""
+    dims = (64, 64, 64, 128)
+    X, Y, Z, T = dims
+    seed = ti.NOISE_SEED
+    F = Fields.from_slabs(dims, True)
+    gauges = {(p, r): F.gauge(p, r) for p in (4, 2) for r in (18, 12)}
+    F.drop_canonical()
+    codes = torch.empty((T, Z, Y, X, 4, 3), dtype=torch.uint8, device="cuda")
+    for t0 in range(0, T, 16):
+        codes[t0:t0 + 16].copy_(torch.from_numpy(ti.z4_codes(dims, seed=seed, t0=t0, t1=t0 + 16)))
+    refs = {}
+    for parity in (0, 1):
+        sites = _sample_sites(dims, parity, 30000, 11 + parity)
+        Uf, Ub, nf, nb, sf, sb = gather_site_inputs(dims, sites, seed, ap=True)
+        d = np.stack([oracle.hop_gathered(Uf[k], Ub[k], nf[k], nb[k], sf[k], sb[k]) for k in range(sites.size)])
+        refs[parity] = (sites, oracle.twist(d.reshape(-1, 1, 1, 1, 4, 3), A, inverse=True).reshape(-1, 4, 3))
+    canon = torch.empty((T * Z * Y * X, 4, 3, 2), dtype=torch.float64, device="cuda")
+    for prec in (4, 2):
+        pin = tm.device_buffer(tm.tm_spinor_bytes(F.L, prec, 1, 1))
+        tm.tm_spinor_pack_z4(F.L, codes, prec, 1, pin)
+        out = tm.device_buffer(tm.tm_spinor_bytes(F.L, prec, 1, 1))
+        for recon in (18, 12):
+            out.zero_()
+            for parity in (0, 1):
+                tm.tm_dslash(F.L, gauges[(prec, recon)], prec, recon, F.half(out, prec, parity), F.half(pin, prec, 1 - parity), None,
+                             parity, 0, tm.TM_KIND_TWIST_INV, KAPPA, MU)
+            tm.tm_spinor_unpack(F.L, out, prec, 1, canon)
+            torch.cuda.synchronize()
+            for parity in (0, 1):
+                sites, ref = refs[parity]
+                got = canon[torch.from_numpy(sites).cuda()].cpu().numpy().view(np.complex128)[..., 0]
+                assert rel(got, ref) < TOL[prec], (prec, recon, parity)
+                # per-site bound as well: no single sampled site may be off by more than 20x the field tolerance
+                worst = np.abs(got - ref).reshape(sites.size, -1).max(axis=1).max() / np.abs(ref).max()
+                assert worst < 20 * TOL[prec], (prec, recon, parity, worst)

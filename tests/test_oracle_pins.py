@@ -321,3 +321,34 @@ def test_P14_stochastic_estimate_converges(U4, dense4):
         errs.append(np.linalg.norm(acc / nr - ref))
     assert errs[1] < 0.6 * errs[0]
     assert errs[1] / np.linalg.norm(ref) < 0.05
+
+
+@pytest.mark.parametrize("dagger", [False, True])
+def test_hop_gathered_is_the_stencil_at_one_site(dagger):
+    """orc_hop_gathered (single-site evaluation used for sampled parity at 64^3x128) against the pinned full-lattice
+    stencil on every site of an antiperiodic 4x4x6x8 lattice, inputs regenerated site by site from the counter-based
+    generators -- and against the free-field closed form H(p) u e^{ipx} of P2 at one site."""
+    import sys, os
+    sys.path.insert(0, os.path.dirname(__file__))
+    from tm_harness import gather_site_inputs
+    dims = (4, 4, 6, 8)
+    X, Y, Z, T = dims
+    U = ti.gauge(dims)
+    psi = ti.z4(dims, seed=91)
+    ref = oracle.hop(U, psi, ap=True, dagger=dagger).reshape(-1, 4, 3)
+    sites = np.arange(X * Y * Z * T)
+    Uf, Ub, nf, nb, sf, sb = gather_site_inputs(dims, sites, 91, ap=True)
+    got = np.stack([oracle.hop_gathered(Uf[k], Ub[k], nf[k], nb[k], sf[k], sb[k], dagger=dagger) for k in sites])
+    assert np.abs(got - ref).max() < 1e-13
+    # free field: U = 1, psi = u e^{ipx}: (Dslash psi)(x) = sum_mu (2 cos p_mu - 2 i E gamma_mu sin p_mu) u e^{ipx}
+    rng = np.random.default_rng(3)
+    u = rng.normal(size=(4, 3)) + 1j * rng.normal(size=(4, 3))
+    p = np.array([2 * np.pi * 1 / X, 2 * np.pi * 3 / Y, 0.0, 2 * np.pi * 2 / T])
+    x = np.array([1, 2, 5, 3])
+    one = np.broadcast_to(np.eye(3, dtype=np.complex128), (4, 3, 3)).copy()
+    nfw = np.stack([u * np.exp(1j * (p @ x + p[mu])) for mu in range(4)])
+    nbw = np.stack([u * np.exp(1j * (p @ x - p[mu])) for mu in range(4)])
+    got1 = oracle.hop_gathered(one, one, nfw, nbw, np.ones(4), np.ones(4), dagger=dagger)
+    E = -1.0 if dagger else 1.0
+    H = sum(2 * np.cos(p[mu]) * np.eye(4) - 2j * E * np.sin(p[mu]) * oracle.gamma(mu) for mu in range(4))
+    assert np.abs(got1 - np.exp(1j * (p @ x)) * (H @ u)).max() < 1e-13

@@ -29,6 +29,27 @@ class Fields:
         self.U_dev = to_dev(U)
         self._gauge = {}
 
+    @classmethod
+    def from_slabs(cls, dims, ap=True, slab=8):
+        """Large lattices: the canonical links are generated and uploaded `slab` time slices at a time (64^3x128 = 19.3 GB)."""
+        import tm_inputs as ti
+        X, Y, Z, T = dims
+        self = cls.__new__(cls)
+        self.dims = tuple(dims)
+        self.L = tm.tm_lattice_create(dims, ap)
+        self.V = self.L.V
+        per_t = X * Y * Z * 4 * 18
+        self.U_dev = torch.empty(T * per_t, dtype=torch.float64, device="cuda")
+        for t0 in range(0, T, slab):
+            t1 = min(T, t0 + slab)
+            self.U_dev[t0 * per_t:t1 * per_t].copy_(torch.from_numpy(ti.gauge(dims, t0=t0, t1=t1).view(np.float64).reshape(-1)))
+        self._gauge = {}
+        return self
+
+    def drop_canonical(self):
+        self.U_dev = None
+        torch.cuda.empty_cache()
+
     def gauge(self, prec, recon):
         key = (prec, recon)
         if key not in self._gauge:
@@ -73,3 +94,32 @@ class Fields:
     def put_half(self, full, stack, prec, parity, nrhs):
         pb = self.pb(prec)
         full.view(nrhs, 2, pb)[:, parity, :].copy_(stack.view(nrhs, pb))
+
+
+def gather_site_inputs(dims, sites, noise_seed, ap=True):
+    """Geometry only: for each global site index x the inputs of the single-site hop (oracle.hop_gathered):
+    U_mu(x), U_mu(x-mu), psi(x+mu), psi(x-mu) from the counter-based generators, and the temporal boundary signs.
+    Returns Ufwd[N][4][3][3], Ubwd[N][4][3][3], nf[N][4][4][3], nb[N][4][4][3], sf[N][4], sb[N][4]."""
+    import tm_inputs as ti
+    X, Y, Z, T = dims
+    sites = np.asarray(sites, dtype=np.int64)
+    c = [sites % X, (sites // X) % Y, (sites // (X * Y)) % Z, sites // (X * Y * Z)]
+    ext = [X, Y, Z, T]
+    stride = [1, X, X * Y, X * Y * Z]
+    N = sites.size
+    Ufwd = ti.gauge_sites(sites)
+    Ubwd = np.empty((N, 4, 3, 3), dtype=np.complex128)
+    nf = np.empty((N, 4, 4, 3), dtype=np.complex128)
+    nb = np.empty((N, 4, 4, 3), dtype=np.complex128)
+    sf = np.ones((N, 4))
+    sb = np.ones((N, 4))
+    for mu in range(4):
+        up = sites + np.where(c[mu] == ext[mu] - 1, -(ext[mu] - 1), 1) * stride[mu]
+        dn = sites + np.where(c[mu] == 0, ext[mu] - 1, -1) * stride[mu]
+        nf[:, mu] = ti.z4_sites(up, seed=noise_seed)
+        nb[:, mu] = ti.z4_sites(dn, seed=noise_seed)
+        Ubwd[:, mu] = ti.gauge_sites(dn)[:, mu]
+    if ap:
+        sf[:, 3] = np.where(c[3] == T - 1, -1.0, 1.0)
+        sb[:, 3] = np.where(c[3] == 0, -1.0, 1.0)
+    return Ufwd, Ubwd, nf, nb, sf, sb
