@@ -261,6 +261,10 @@ def run_b200(args, rank, world, local_rank):
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
     if rank == 0:
         extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world)
+        if args.sweeps and world == 1:
+            del gauges, eta, sol, cg_ws, tsm_ws
+            torch.cuda.empty_cache()
+            sweep_other_configs(torch, tm, ti, hbm_peak, out)
         print(json.dumps(out))
     if world > 1:
         dist.barrier()
@@ -347,12 +351,104 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
         out["cpu_baseline"] = base
 
 
+def sweep_other_configs(torch, tm, ti, hbm_peak, out):
+    """`--sweeps`: BASELINE.json configs[1] (16^3x32 fp32, 100 applications captured in a CUDA graph: L2 / launch-latency
+    regime, NOT an HBM roofline point) and configs[4] (64^3x128: the clean HBM-bound sweep, working set >> L2)."""
+    kappa, mu = ti.KAPPA, ti.MU
+    # ---- configs[1] ----
+    dims = (16, 16, 16, 32)
+    L = tm.tm_lattice_create(dims, True)
+    Vh = L.V // 2
+    U = torch.from_numpy(ti.gauge(dims).view(np.float64)).cuda()
+    psi = torch.from_numpy(ti.z4(dims).view(np.float64)).cuda()
+    small = {}
+    prec = 4
+    pb = tm.tm_spinor_bytes(L, prec, 0, 1)
+    src = tm.device_buffer(2 * pb)
+    tm.tm_spinor_pack(L, psi, prec, 1, src)
+    a, b, tmp = tm.device_buffer(pb), tm.device_buffer(pb), tm.device_buffer(2 * pb)
+    for recon in (18, 12):
+        g = tm.device_buffer(tm.tm_gauge_bytes(L, prec, recon))
+        tm.tm_gauge_pack(L, U, prec, recon, g, 1e-10)
+        for name, fl, by in (("twist_inv", FLOPS_TWIST_INV, dslash_bytes(Vh, prec, recon, False)),
+                             ("MdagM", 2 * (FLOPS_TWIST_INV + FLOPS_XPAY), 2 * dslash_bytes(Vh, prec, recon, False) + 2 * dslash_bytes(Vh, prec, recon, True))):
+            st = torch.cuda.Stream()
+            def body():
+                for i in range(100):
+                    o, inp = (a, b) if i % 2 == 0 else (b, a)
+                    if name == "twist_inv":
+                        tm.tm_dslash(L, g, prec, recon, o, src[pb:2 * pb] if i == 0 else inp, None, 0, 0, tm.TM_KIND_TWIST_INV, kappa, mu)
+                    else:
+                        tm.tm_MdagM(L, g, prec, recon, o, src[:pb] if i == 0 else inp, tmp, 0, kappa, mu)
+            with torch.cuda.stream(st):
+                body()  # warm-up (also loads the modules before capture)
+                st.synchronize()
+                graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(graph, stream=st):
+                    body()
+                ts = []
+                for _ in range(5):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(st); graph.replay(); e1.record(st); st.synchronize()
+                    ts.append(e0.elapsed_time(e1) / 100)
+            ms = float(np.median(ts))
+            small["%s_fp32_recon%d" % (name, recon)] = {"us": ms * 1e3, "GFLOPS": Vh * fl / ms / 1e6, "GBps_algorithmic": by / ms / 1e6}
+    out["config1_16x32_fp32_graph"] = {"note": "L2-resident working set (<= 50 MB), 100 applications in one CUDA graph, median of 5: "
+                                       "L2 / launch-latency regime, not an HBM roofline point", "table": small}
+    del U, psi, src, a, b, tmp
+    # ---- configs[4] ----
+    dims = (64, 64, 64, 128)
+    X, Y, Z, T = dims
+    L = tm.tm_lattice_create(dims, True)
+    Vh = L.V // 2
+    per_t = X * Y * Z * 4 * 18
+    U = torch.empty(T * per_t, dtype=torch.float64, device="cuda")
+    for t0 in range(0, T, 8):
+        U[t0 * per_t:(t0 + 8) * per_t].copy_(torch.from_numpy(ti.gauge(dims, t0=t0, t1=t0 + 8).view(np.float64).reshape(-1)))
+    gauges = {}
+    for prec in (4, 2):
+        for recon in (18, 12):
+            gauges[(prec, recon)] = tm.device_buffer(tm.tm_gauge_bytes(L, prec, recon))
+            tm.tm_gauge_pack(L, U, prec, recon, gauges[(prec, recon)], 1e-10)
+    del U
+    torch.cuda.empty_cache()
+    codes = torch.empty((T, Z, Y, X, 4, 3), dtype=torch.uint8, device="cuda")
+    for t0 in range(0, T, 16):
+        codes[t0:t0 + 16].copy_(torch.from_numpy(ti.z4_codes(dims, t0=t0, t1=t0 + 16)))
+    big = {}
+    for prec in (4, 2):
+        pb = tm.tm_spinor_bytes(L, prec, 0, 1)
+        src = tm.device_buffer(2 * pb)
+        tm.tm_spinor_pack_z4(L, codes, prec, 1, src)
+        o, x, tmp = tm.device_buffer(pb), tm.device_buffer(pb), tm.device_buffer(2 * pb)
+        x.copy_(src[:pb])
+        for recon in (18, 12):
+            g = gauges[(prec, recon)]
+            runs = (("twist_inv", FLOPS_TWIST_INV, dslash_bytes(Vh, prec, recon, False),
+                     lambda i: tm.tm_dslash(L, g, prec, recon, o, src[pb:2 * pb], None, 0, 0, tm.TM_KIND_TWIST_INV, kappa, mu)),
+                    ("xpay_twist", FLOPS_XPAY, dslash_bytes(Vh, prec, recon, True),
+                     lambda i: tm.tm_dslash(L, g, prec, recon, o, src[pb:2 * pb], x, 0, 0, tm.TM_KIND_XPAY_TWIST, kappa, mu)),
+                    ("MdagM", 2 * (FLOPS_TWIST_INV + FLOPS_XPAY), 2 * dslash_bytes(Vh, prec, recon, False) + 2 * dslash_bytes(Vh, prec, recon, True),
+                     lambda i: tm.tm_MdagM(L, g, prec, recon, o, src[:pb], tmp, 0, kappa, mu)))
+            for name, fl, by, fn in runs:
+                for i in range(3):
+                    fn(i)
+                ms = min(time_events(torch, fn, 10) for _ in range(3))
+                big["%s_fp%d_recon%d" % (name, prec * 8, recon)] = {
+                    "us": ms * 1e3, "GFLOPS": Vh * fl / ms / 1e6, "GBps_algorithmic": by / ms / 1e6,
+                    "frac_of_measured_%.0f" % hbm_peak: by / ms / 1e6 / hbm_peak, "frac_of_nominal_8000": by / ms / 1e6 / 8000.0}
+        del src, o, x, tmp
+    out["config4_64x128"] = {"note": "33.5 M sites; gauge 3.2-9.7 GB + spinors 0.9-1.6 GB per parity: every launch streams from HBM",
+                             "table": big}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--sweeps", action="store_true", help="also time BASELINE.json configs[1] (16^3x32, CUDA graph) and [4] (64^3x128)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
