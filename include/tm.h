@@ -149,6 +149,36 @@ size_t tm_loop_workspace_bytes(const tm_lattice* L, int nrhs);
 int tm_loop_contract(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, double* out,
                      void* workspace, void* stream);
 
+/* ---- NEXT-1: estimators built from the rows above ------------------------------------------ */
+/* a8': out[rhs][n][t] = scale * sum_{x: x4=t} (g5^g5_left a)^dag (Gamma_n x 1) (g5^g5_right b), scale = scale_re + i scale_im.
+ * g5 = diag(1,1,-1,-1) in the public basis.  Same buffers and workspace as tm_loop_contract (which is g5 flags 0, scale 1). */
+int tm_loop_contract_ex(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, int g5_left,
+                        int g5_right, double scale_re, double scale_im, double* out, void* workspace, void* stream);
+
+/* Full (unpreconditioned) operator on packed full-lattice spinors [nrhs][parity][...]:
+ *   out = M(kappa, mu) in = (1 + i 2 kappa mu g5) in - kappa Dslash in   (M^dag if dagger).  mu = 0: the Wilson operator
+ *   D_W = (M_u + M_d)/2 of PAPER.md:137 Eq. (14).  out_full must not alias in_full.  Two fused dslash launches. */
+int tm_M(const tm_lattice* L, const void* gauge, int prec, int recon, void* out_full, const void* in_full, double kappa,
+         double mu, int dagger, int nrhs, void* stream);
+
+/* One-end trick loops from solutions s = M(kappa,+mu)^-1 eta, s_full: DEVICE [nrhs][parity][...]:
+ *   TM_ONEEND_TAU3:    out[rhs][n][t] = 2 i (2 kappa mu) sum_{x: x4=t} s^dag g5 Gamma_n s             (Eq. 13; gauge may be NULL)
+ *   TM_ONEEND_GENERAL: out[rhs][n][t] = 2 sum_{x: x4=t} s^dag g5 Gamma_n g5 D_W s, D_W = M(kappa,0)   (Eq. 15)
+ * Noise averages (kappa-normalised M, readings 1, 25): TAU3 -> Tr_t[M_d^-1 Gamma_n] - Tr_t[M_u^-1 Gamma_n] (the sign
+ * printed in Eq. 13 belongs to s = M_d^-1 eta), GENERAL -> Tr_t[M_u^-1 Gamma_n] + Tr_t[M_d^-1 Gamma_n].
+ * out: DEVICE double [nrhs][16][T][2]; workspace: DEVICE, tm_oneend_workspace_bytes(). */
+typedef enum { TM_ONEEND_TAU3 = 0, TM_ONEEND_GENERAL = 1 } tm_oneend_kind;
+size_t tm_oneend_workspace_bytes(const tm_lattice* L, int prec, int nrhs);
+int tm_oneend_loops(const tm_lattice* L, const void* gauge, int prec, int recon, const void* s_full, int kind, double kappa,
+                    double mu, int nrhs, double* out, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Truncated-solver-method combination, Eq. (8), applied to loops:
+ *   out[n][t] = 1/n_hp sum_{r<n_hp} (loops_hp[r] - loops_lp_same[r]) + 1/n_lp sum_{j<n_lp} loops_lp[j]
+ * loops_hp / loops_lp_same: the HP and LP loops of the SAME n_hp sources; loops_lp: the n_lp further LP sources.
+ * All DEVICE double [count][16][T][2]; out DEVICE double [16][T][2].  Fixed summation order. */
+int tm_tsm_combine(int T, const double* loops_hp, const double* loops_lp_same, int n_hp, const double* loops_lp, int n_lp,
+                   double* out, void* stream);
+
 /* ---- end-to-end TSM batch with HOST buffers ("the source is sent to the GPUs for inversion and
  *      contraction, and contractions are stored back in the CPUs") ----------------------------------------- */
 /* codes_host: HOST (pinned recommended) uint8 [nrhs][V][12] Z2xiZ2 codes; loops_host: HOST double [nrhs][16][T][2].

@@ -159,3 +159,38 @@ def loop(a, b):
     out = np.empty((16, T), dtype=np.complex128)
     _load().orc_loop(_dims(a), a.ctypes.data, b.ctypes.data, out.ctypes.data)
     return out
+
+
+# ---- NEXT-1: estimators, written out in the paper's order -------------------------------------
+
+def gamma5(psi):
+    """g5 psi with g5 = gamma(4) = g1 g2 g3 g4 as a full 4x4 matrix acting on the spin index."""
+    return np.einsum("ab,...bc->...ac", gamma(4), _c(psi))
+
+
+def loop_oneend_tau3(s, kappa, mu):
+    """PAPER.md:127 Eq. (13), kappa-normalised (2 mu a -> 2 (2 kappa mu)): 2 i (2 kappa mu) sum_x s^dag g5 Gamma_n s, [16][T]."""
+    return 2j * (2 * kappa * mu) * loop(gamma5(s), s)
+
+
+def loop_oneend_general(U, s, kappa, ap=True):
+    """PAPER.md:141 Eq. (15): 2 sum_x s^dag g5 Gamma_n g5 D_W s with D_W = (M_u + M_d)/2 = M(kappa, 0) (Eq. 14)."""
+    DWs = M(U, s, kappa, 0.0, ap=ap)
+    return 2.0 * loop(gamma5(s), gamma5(DWs))
+
+
+def tsm_combine(L_hp, L_lp_same, L_lp):
+    """PAPER.md:75-77 Eq. (8) applied to loops: 1/N_HP sum_r [L_HP(r) - L_LP(r)] + 1/N_LP sum_j L_LP(j).
+    L_hp, L_lp_same: [N_HP][16][T] of the same sources; L_lp: [N_LP][16][T]."""
+    out = 0
+    if len(L_hp):
+        c = 0
+        for r in range(len(L_hp)):
+            c = c + (L_hp[r] - L_lp_same[r])
+        out = out + c / len(L_hp)
+    if len(L_lp):
+        l = 0
+        for j in range(len(L_lp)):
+            l = l + L_lp[j]
+        out = out + l / len(L_lp)
+    return out

@@ -12,6 +12,7 @@ TM_PREC_F64, TM_PREC_F32, TM_PREC_F16 = 8, 4, 2
 TM_RECON_18, TM_RECON_12 = 18, 12
 TM_KIND_PLAIN, TM_KIND_TWIST_INV, TM_KIND_XPAY_TWIST = 0, 1, 2
 TM_CG_HP_MIXED, TM_CG_LP_TRUNCATED = 0, 1
+TM_ONEEND_TAU3, TM_ONEEND_GENERAL = 0, 1
 TM_OK, TM_ERR_ARG, TM_ERR_LAYOUT, TM_ERR_NOT_SU3, TM_ERR_CUDA, TM_ERR_BREAKDOWN, TM_ERR_MAXITER = 0, -1, -2, -3, -4, -5, -6
 TM_MAX_NRHS = 16
 
@@ -19,7 +20,8 @@ ABI_SYMBOLS = [
     "tm_version", "tm_strerror", "tm_last_cuda_error", "tm_lattice_create", "tm_lattice_destroy", "tm_gauge_bytes",
     "tm_spinor_bytes", "tm_gauge_pack", "tm_spinor_pack", "tm_spinor_unpack", "tm_spinor_pack_z4", "tm_dslash",
     "tm_dslash_general", "tm_MdagM", "tm_cg_workspace_bytes", "tm_cg_multi", "tm_cg", "tm_loop_workspace_bytes",
-    "tm_loop_contract", "tm_tsm_workspace_bytes", "tm_tsm_batch_host", "tm_launch_count", "tm_kernel_timing_enable",
+    "tm_loop_contract", "tm_loop_contract_ex", "tm_M", "tm_oneend_workspace_bytes", "tm_oneend_loops", "tm_tsm_combine",
+    "tm_tsm_workspace_bytes", "tm_tsm_batch_host", "tm_launch_count", "tm_kernel_timing_enable",
     "tm_kernel_timing_read",
 ]
 
@@ -77,6 +79,11 @@ def load():
         "tm_cg": (i, [vp, vp, i, vp, i, i, vp, vp, P(tm_cg_params), P(tm_cg_info), vp, sz, vp]),
         "tm_loop_workspace_bytes": (sz, [vp, i]),
         "tm_loop_contract": (i, [vp, vp, vp, i, i, vp, vp, vp]),
+        "tm_loop_contract_ex": (i, [vp, vp, vp, i, i, i, i, d, d, vp, vp, vp]),
+        "tm_M": (i, [vp, vp, i, i, vp, vp, d, d, i, i, vp]),
+        "tm_oneend_workspace_bytes": (sz, [vp, i, i]),
+        "tm_oneend_loops": (i, [vp, vp, i, i, vp, i, d, d, i, vp, vp, sz, vp]),
+        "tm_tsm_combine": (i, [i, vp, vp, i, vp, i, vp, vp]),
         "tm_tsm_workspace_bytes": (sz, [vp, i, i]),
         "tm_tsm_batch_host": (i, [vp, vp, i, i, vp, P(tm_cg_params), i, P(tm_cg_info), vp, vp, sz, vp]),
         "tm_launch_count": (ctypes.c_ulonglong, []),
@@ -227,6 +234,32 @@ def tm_loop_workspace_bytes(L, nrhs=1):
 def tm_loop_contract(L, a_full, b_full, prec, nrhs, out, workspace, stream=None):
     return _check(load().tm_loop_contract(L.handle, _ptr(a_full), _ptr(b_full), prec, nrhs, _ptr(out), _ptr(workspace), _stream(stream)),
                   "tm_loop_contract")
+
+
+def tm_loop_contract_ex(L, a_full, b_full, prec, nrhs, g5_left, g5_right, scale, out, workspace, stream=None):
+    scale = complex(scale)
+    return _check(load().tm_loop_contract_ex(L.handle, _ptr(a_full), _ptr(b_full), prec, nrhs, int(g5_left), int(g5_right), scale.real,
+                                             scale.imag, _ptr(out), _ptr(workspace), _stream(stream)), "tm_loop_contract_ex")
+
+
+def tm_M(L, gauge, prec, recon, out_full, in_full, kappa, mu, dagger=0, nrhs=1, stream=None):
+    return _check(load().tm_M(L.handle, _ptr(gauge), prec, recon, _ptr(out_full), _ptr(in_full), kappa, mu, int(dagger), nrhs,
+                              _stream(stream)), "tm_M")
+
+
+def tm_oneend_workspace_bytes(L, prec, nrhs=1):
+    return load().tm_oneend_workspace_bytes(L.handle, prec, nrhs)
+
+
+def tm_oneend_loops(L, gauge, prec, recon, s_full, kind, kappa, mu, nrhs, out, workspace, stream=None):
+    ws_bytes = workspace.numel() * workspace.element_size()
+    return _check(load().tm_oneend_loops(L.handle, _ptr(gauge), prec, recon, _ptr(s_full), kind, kappa, mu, nrhs, _ptr(out),
+                                         _ptr(workspace), ws_bytes, _stream(stream)), "tm_oneend_loops")
+
+
+def tm_tsm_combine(T, loops_hp, loops_lp_same, n_hp, loops_lp, n_lp, out, stream=None):
+    return _check(load().tm_tsm_combine(T, _ptr(loops_hp), _ptr(loops_lp_same), n_hp, _ptr(loops_lp), n_lp, _ptr(out),
+                                        _stream(stream)), "tm_tsm_combine")
 
 
 def tm_tsm_workspace_bytes(L, prec_lp, nrhs):

@@ -94,6 +94,8 @@ int spinor_pack_any(const Geo& g, long long V, int prec, int mode, const double*
                     void* packed, int nrhs, cudaStream_t st);
 int loop_contract(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,
                   cudaStream_t st);
+int loop_contract_ex(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,
+                     int g5_left, int g5_right, double scale_re, double scale_im, cudaStream_t st);
 size_t loop_workspace_bytes(const Geo& g, int nrhs);
 void kernel_timing_begin(cudaStream_t st);
 void kernel_timing_end(cudaStream_t st);

@@ -6,8 +6,8 @@
 // obtained, with enough information to reconstruct any arbitrary gamma insertion") followed by
 // L[n][t] = sum_{al be} (Gamma_n)_{al be} C_{al be}(t).
 // Time slice t of parity p is the contiguous checkerboard range [t*V3h, (t+1)*V3h).
-// Reduction: per-site products in the storage arithmetic (fp32 for fp32/fp16 inputs), accumulated in fp64 per
-// thread, warp shuffles, shared memory across warps, per-block partials, then one fixed-order final pass:
+// Reduction: per-site products in the storage arithmetic (fp32 for fp32/fp16 inputs), summed in that arithmetic over
+// at most LOOP_CHUNK = 8 sites of a thread, then fp64: per-thread accumulator, warp shuffles, shared memory across warps, per-block partials, then one fixed-order final pass:
 // bit-reproducible, no floating-point atomics.
 #include "tm_layout.cuh"
 
@@ -62,6 +62,7 @@ static GammaTable make_gamma_table()
 }
 
 constexpr int LOOP_THREADS = 128;
+constexpr int LOOP_CHUNK = 8; // sites summed in the storage arithmetic before the fp64 accumulator takes over
 
 template <int PREC>
 __global__ void __launch_bounds__(LOOP_THREADS) loop_partial_kernel(Geo g, const char* a_full, const char* b_full,
@@ -71,10 +72,16 @@ __global__ void __launch_bounds__(LOOP_THREADS) loop_partial_kernel(Geo g, const
     const int t = blockIdx.y, rhs = blockIdx.z;
     const char* af = a_full + (size_t)rhs * 2 * parity_bytes;
     const char* bf = b_full + (size_t)rhs * 2 * parity_bytes;
+    // per-thread partial sums: products and the sum over up to LOOP_CHUNK sites in the storage arithmetic, then fp64
     double acc[32];
+    real accf[32];
 #pragma unroll
-    for (int k = 0; k < 32; ++k) acc[k] = 0.0;
+    for (int k = 0; k < 32; ++k) {
+        acc[k] = 0.0;
+        accf[k] = 0;
+    }
     const int nsite = 2 * g.V3h;
+    int pending = 0;
     for (int i = blockIdx.x * LOOP_THREADS + threadIdx.x; i < nsite; i += nb * LOOP_THREADS) {
         const int parity = i >= g.V3h;
         const int cb = t * g.V3h + (i - parity * g.V3h);
@@ -85,7 +92,7 @@ __global__ void __launch_bounds__(LOOP_THREADS) loop_partial_kernel(Geo g, const
         for (int al = 0; al < 4; ++al)
 #pragma unroll
             for (int be = 0; be < 4; ++be) {
-                real re = 0, im = 0;
+                real re = accf[(al * 4 + be) * 2], im = accf[(al * 4 + be) * 2 + 1];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     const real ar = a[(al * 3 + c) * 2], ai = a[(al * 3 + c) * 2 + 1];
@@ -95,10 +102,20 @@ __global__ void __launch_bounds__(LOOP_THREADS) loop_partial_kernel(Geo g, const
                     im = fma(ar, bi, im);
                     im = fma(-ai, br, im);
                 }
-                acc[(al * 4 + be) * 2] += (double)re;
-                acc[(al * 4 + be) * 2 + 1] += (double)im;
+                accf[(al * 4 + be) * 2] = re;
+                accf[(al * 4 + be) * 2 + 1] = im;
             }
+        if (++pending == LOOP_CHUNK) {
+#pragma unroll
+            for (int k = 0; k < 32; ++k) {
+                acc[k] += (double)accf[k];
+                accf[k] = 0;
+            }
+            pending = 0;
+        }
     }
+#pragma unroll
+    for (int k = 0; k < 32; ++k) acc[k] += (double)accf[k];
     __shared__ double sm[LOOP_THREADS / 32][32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
@@ -117,7 +134,10 @@ __global__ void __launch_bounds__(LOOP_THREADS) loop_partial_kernel(Geo g, const
     }
 }
 
-__global__ void loop_final_kernel(int T, int nb, const double* partial, GammaTable tb, double* out)
+// out = scale * sum_{al be} (Gamma_n)_{al be} s5(al)^g5_left s5(be)^g5_right C_{al be}(t), s5 = (1,1,-1,-1) = diag g5:
+// the bilinear (g5^l a)^dag Gamma_n (g5^r b) of the one-end trick (PAPER.md:127 Eq. 13, :141 Eq. 15)
+__global__ void loop_final_kernel(int T, int nb, const double* partial, GammaTable tb, double* out, int g5_left, int g5_right,
+                                  double scale_re, double scale_im)
 {
     const int t = blockIdx.x, rhs = blockIdx.y;
     __shared__ double C[32];
@@ -135,12 +155,13 @@ __global__ void loop_final_kernel(int T, int nb, const double* partial, GammaTab
         for (int al = 0; al < 4; ++al) {
             const int be = tb.col[n][al];
             const double gr = tb.re[n][al], gi = tb.im[n][al];
-            const double cr = C[(al * 4 + be) * 2], ci = C[(al * 4 + be) * 2 + 1];
+            const double sg = ((g5_left && al >= 2) ? -1.0 : 1.0) * ((g5_right && be >= 2) ? -1.0 : 1.0);
+            const double cr = sg * C[(al * 4 + be) * 2], ci = sg * C[(al * 4 + be) * 2 + 1];
             re += gr * cr - gi * ci;
             im += gr * ci + gi * cr;
         }
-        out[(((size_t)rhs * 16 + n) * T + t) * 2] = re;
-        out[(((size_t)rhs * 16 + n) * T + t) * 2 + 1] = im;
+        out[(((size_t)rhs * 16 + n) * T + t) * 2] = scale_re * re - scale_im * im;
+        out[(((size_t)rhs * 16 + n) * T + t) * 2 + 1] = scale_re * im + scale_im * re;
     }
 }
 
@@ -152,8 +173,8 @@ static int loop_nb(const Geo& g)
     return nb;
 }
 
-int loop_contract(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,
-                  cudaStream_t st)
+int loop_contract_ex(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,
+                     int g5_left, int g5_right, double scale_re, double scale_im, cudaStream_t st)
 {
     static const GammaTable tb = make_gamma_table();
     const int nb = loop_nb(g);
@@ -164,9 +185,15 @@ int loop_contract(const Geo& g, const void* a_full, const void* b_full, int prec
     else if (prec == 4) loop_partial_kernel<4><<<grid, block, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, partial, nb);
     else loop_partial_kernel<2><<<grid, block, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, partial, nb);
     TM_LAUNCH_CHECK("loop_partial_kernel");
-    loop_final_kernel<<<dim3(g.T, nrhs), 32, 0, st>>>(g.T, nb, partial, tb, out);
+    loop_final_kernel<<<dim3(g.T, nrhs), 32, 0, st>>>(g.T, nb, partial, tb, out, g5_left, g5_right, scale_re, scale_im);
     TM_LAUNCH_CHECK("loop_final_kernel");
     return TM_OK;
+}
+
+int loop_contract(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,
+                  cudaStream_t st)
+{
+    return loop_contract_ex(g, a_full, b_full, prec, nrhs, out, workspace, 0, 0, 1.0, 0.0, st);
 }
 
 size_t loop_workspace_bytes(const Geo& g, int nrhs) { return round256((size_t)nrhs * g.T * loop_nb(g) * 32 * sizeof(double)); }
@@ -187,4 +214,13 @@ extern "C" int tm_loop_contract(const tm_lattice* L, const void* a_full, const v
     if (!L || !a_full || !b_full || !out || !workspace || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
     if (!aligned256(a_full) || !aligned256(b_full) || !aligned256(out) || !aligned256(workspace)) return TM_ERR_LAYOUT;
     return loop_contract(L->g, a_full, b_full, prec, nrhs, out, workspace, (cudaStream_t)stream);
+}
+
+extern "C" int tm_loop_contract_ex(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, int g5_left,
+                                   int g5_right, double scale_re, double scale_im, double* out, void* workspace, void* stream)
+{
+    if (!L || !a_full || !b_full || !out || !workspace || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
+    if (!aligned256(a_full) || !aligned256(b_full) || !aligned256(out) || !aligned256(workspace)) return TM_ERR_LAYOUT;
+    return loop_contract_ex(L->g, a_full, b_full, prec, nrhs, out, workspace, g5_left != 0, g5_right != 0, scale_re, scale_im,
+                            (cudaStream_t)stream);
 }

@@ -352,3 +352,40 @@ def test_hop_gathered_is_the_stencil_at_one_site(dagger):
     E = -1.0 if dagger else 1.0
     H = sum(2 * np.cos(p[mu]) * np.eye(4) - 2j * E * np.sin(p[mu]) * oracle.gamma(mu) for mu in range(4))
     assert np.abs(got1 - np.exp(1j * (p @ x)) * (H @ u)).max() < 1e-13
+
+
+def test_P17_one_end_trick_exact_traces(U4, dense4):
+    """PAPER.md:120-141 Eq. (11)-(15) as exact identities on 4^4: summing the one-end loops over ALL 3072 unit sources
+    (s_i = column i of the dense inverse) gives Tr_t[(M_d^-1 - M_u^-1) Gamma_n] (tau3 form, s = M_u^-1 eta; DESIGN.md
+    reading 25 on the sign) and Tr_t[(M_u^-1 + M_d^-1) Gamma_n] (generalised form)."""
+    dims = (4, 4, 4, 4)
+    _, Su = dense4
+    Sd = np.linalg.inv(dense.dense_M(U4, KAPPA, -MU, ap=True))
+    tr_u, tr_d = dense.timeslice_traces(Su, dims), dense.timeslice_traces(Sd, dims)
+    acc3 = np.zeros((16, 4), dtype=np.complex128)
+    accg = np.zeros((16, 4), dtype=np.complex128)
+    for i in range(Su.shape[1]):
+        s = Su[:, i].reshape(4, 4, 4, 4, 4, 3)
+        acc3 += oracle.loop_oneend_tau3(s, KAPPA, MU)
+        accg += oracle.loop_oneend_general(U4, s, KAPPA)
+    assert np.abs(acc3 - (tr_d - tr_u)).max() < 1e-11 * max(1.0, np.abs(tr_u).max())
+    assert np.abs(accg - (tr_u + tr_d)).max() < 1e-10 * np.abs(tr_u).max()
+    # gamma5 of the oracle is the diagonal (1,1,-1,-1) of the declared basis and squares to one
+    psi = ti.gauss_spinor(dims, 4)
+    assert np.array_equal(oracle.gamma5(psi), psi * np.array([1, 1, -1, -1])[:, None])
+
+
+def test_P18_tsm_combination_closed_forms():
+    """PAPER.md:75-77 Eq. (8): constants c1, c2, c3 give c1 - c2 + c3; identical HP/LP pairs leave the LP mean; N_LP = 0
+    leaves the mean correction; the combination is linear."""
+    rng = np.random.default_rng(8)
+    shp = (16, 6)
+    c1, c2, c3 = (rng.normal(size=shp) + 1j * rng.normal(size=shp) for _ in range(3))
+    out = oracle.tsm_combine([c1] * 3, [c2] * 3, [c3] * 5)
+    assert np.abs(out - (c1 - c2 + c3)).max() < 1e-14
+    hp = rng.normal(size=(4,) + shp) + 0j
+    lp = rng.normal(size=(7,) + shp) + 0j
+    assert np.abs(oracle.tsm_combine(hp, hp, lp) - lp.mean(axis=0)).max() < 1e-14
+    lps = rng.normal(size=(4,) + shp) + 0j
+    assert np.abs(oracle.tsm_combine(hp, lps, lp[:0]) - (hp - lps).mean(axis=0)).max() < 1e-14
+    assert np.abs(oracle.tsm_combine(2 * hp, 2 * lps, 2 * lp) - 2 * oracle.tsm_combine(hp, lps, lp)).max() < 1e-13
