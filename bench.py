@@ -10,7 +10,7 @@ fp32 / fp16 x 18 / 12 reals (configs[2]), and a mixed-precision CG to 1e-8.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
 N > 1: launched under torch.distributed.run; noise sources are independent, so ranks take different batches and
-there is no data-path collective (weak scaling, "replicas + gather" of the [16][T] loops).
+there is no data-path collective (weak scaling, "replicas + gather" of the [16][T] loops through paper_1309_2256_b200.shard).
 """
 import argparse
 import json
@@ -140,6 +140,7 @@ def run_b200(args, rank, world, local_rank):
     import torch.distributed as dist
     import tm_inputs as ti
     import paper_1309_2256_b200 as tm
+    from paper_1309_2256_b200 import shard
     tm.load()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
@@ -182,6 +183,8 @@ def run_b200(args, rank, world, local_rank):
         rc, info = tm.tm_cg_multi(L, None, 8, g_lp, prec, recon, sol, eta, prm, NRHS, cg_ws)
         assert rc == tm.TM_OK, rc
         tm.tm_loop_contract(L, eta, sol, prec, NRHS, loops, loop_ws)
+        if world > 1:  # the path's only exchange: one gather of the [16][T] loops (16 KB per source), SURVEY.md 8(e)
+            shard.gather_loops(loops, world * NRHS, NRHS)
         iters_log.append([x.iters for x in info])
 
     def step_e2e(i):
@@ -257,7 +260,7 @@ def run_b200(args, rank, world, local_rank):
                                   "12-real links, 12 RHS per gauge load, + 16-Gamma per-timeslice loop of each solution",
                       "lattice": list(DIMS), "kappa": kappa, "mu": mu, "gauge": "seeded SU(3), eps=0.5", "nrhs": NRHS,
                       "iters_per_solve": float(np.mean(iters_log)), "l2": "inputs larger than L2 (gauge 201 MB + 12x2x54.5 MB vectors)",
-                      "parallelism": "independent noise batches per GPU (no collective)"},
+                      "parallelism": "independent noise batches per GPU; one all_gather of the loops per step (16 KB per source)"},
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
     if rank == 0:
         extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world)
