@@ -54,6 +54,25 @@ int launch_dslash_t(const Geo& g, const DslashParams& p, cudaStream_t st);
 TM_DECL(8, 18) TM_DECL(8, 12) TM_DECL(4, 18) TM_DECL(4, 12) TM_DECL(2, 18) TM_DECL(2, 12)
 #undef TM_DECL
 
+template <int PREC, int RECON>
+int link_cache_build_t(const Geo& g, const void* gauge, void* cache, cudaStream_t st);
+#define TM_DECL_LC(P, R) template <> int link_cache_build_t<P, R>(const Geo&, const void*, void*, cudaStream_t);
+TM_DECL_LC(4, 18) TM_DECL_LC(4, 12) TM_DECL_LC(2, 18) TM_DECL_LC(2, 12)
+
+// sizeof(TileSmem<32>) = 8*32*4 + 8*4*32*16 + 8*32*8 bytes per 32-site tile, both parities
+size_t link_cache_bytes(const Geo& g, int prec)
+{
+    if (prec == 8) return 0;
+    return round256((size_t)2 * ((g.Vh + 31) / 32) * 19456);
+}
+
+int link_cache_build(const Geo& g, int prec, int recon, const void* gauge, void* cache, cudaStream_t st)
+{
+    if (prec == 4) return recon == 18 ? link_cache_build_t<4, 18>(g, gauge, cache, st) : link_cache_build_t<4, 12>(g, gauge, cache, st);
+    if (prec == 2) return recon == 18 ? link_cache_build_t<2, 18>(g, gauge, cache, st) : link_cache_build_t<2, 12>(g, gauge, cache, st);
+    return TM_ERR_ARG;
+}
+
 int launch_dslash(const Geo& g, int prec, int recon, const DslashParams& p, cudaStream_t st)
 {
     if (prec == 8) return recon == 18 ? launch_dslash_t<8, 18>(g, p, st) : launch_dslash_t<8, 12>(g, p, st);
@@ -193,13 +212,13 @@ namespace tmk {
 // M_pc^dag M_pc on `parity` with explicit strides/active flags (shared by tm_MdagM and the CG driver)
 int mdagm_apply(const Geo& g, const void* gauge, int prec, int recon, void* out, size_t out_stride, const void* in,
                 size_t in_stride, void* tmp, int parity, double kappa, double mu, int nrhs, const unsigned char* active,
-                cudaStream_t st)
+                cudaStream_t st, const void* link_cache)
 {
     const size_t pb = spinor_parity_bytes(g, prec);
     char* t1 = static_cast<char*>(tmp);
     char* t2 = t1 + pb * nrhs;
     DslashParams p;
-    p.gauge = gauge; p.nrhs = nrhs; p.active = active;
+    p.gauge = gauge; p.nrhs = nrhs; p.active = active; p.link_cache = link_cache;
     p.rhs_stride_out = p.rhs_stride_in = p.rhs_stride_x = pb;
     int rc;
     // t1 = R^-1 D_{pbar p} in

@@ -70,9 +70,10 @@ static int k_axpby(const Geo& g, int py, int px, VecArg y, VecArg x, double a, d
 }
 
 static int k_cg_iter(const Geo& g, const void* gauge, int prec, int recon, VecArg x, VecArg r, VecArg p, VecArg Ap, void* tmp,
-                     double kappa, double mu, const BlasCtx& c, int nrhs, bool do_update_p, cudaStream_t st)
+                     double kappa, double mu, const BlasCtx& c, int nrhs, bool do_update_p, cudaStream_t st,
+                     const void* link_cache = nullptr)
 {
-    int rc = mdagm_apply(g, gauge, prec, recon, Ap.p, Ap.stride, p.p, p.stride, tmp, 0, kappa, mu, nrhs, c.active, st);
+    int rc = mdagm_apply(g, gauge, prec, recon, Ap.p, Ap.stride, p.p, p.stride, tmp, 0, kappa, mu, nrhs, c.active, st, link_cache);
     if (rc != TM_OK) return rc;
     dim3 grid(blas_blocks(g.Vh), nrhs);
     return by_prec(prec, [&](auto P) {
@@ -147,7 +148,7 @@ static int init_ctx(const BlasCtx& c, const tm_cg_params* p, int nrhs, cudaStrea
 
 // b'' (stride pb) from the full-lattice source; t1, t2: scratch (stride pb)
 static int prepare_rhs(const Geo& g, const void* gauge, int prec, int recon, const void* eta_full, void* b, void* t1, void* t2,
-                       double kappa, double mu, int nrhs, cudaStream_t st)
+                       double kappa, double mu, int nrhs, cudaStream_t st, const void* link_cache = nullptr)
 {
     const size_t pb = spinor_parity_bytes(g, prec);
     const char* eta_e = static_cast<const char*>(eta_full);
@@ -157,7 +158,7 @@ static int prepare_rhs(const Geo& g, const void* gauge, int prec, int recon, con
     // t1 = R^-1 eta_o
     if ((rc = k_twist(g, prec, V_(t1, pb), V_(eta_o, 2 * pb), n, -a * n, nrhs, st)) != TM_OK) return rc;
     DslashParams p;
-    p.gauge = gauge; p.nrhs = nrhs; p.active = nullptr;
+    p.gauge = gauge; p.nrhs = nrhs; p.active = nullptr; p.link_cache = link_cache;
     // t2 = b' = eta_e + kappa D_eo t1
     p.out = t2; p.in = t1; p.x = eta_e; p.out_parity = 0; p.dagger = 0;
     p.rhs_stride_out = pb; p.rhs_stride_in = pb; p.rhs_stride_x = 2 * pb;
@@ -175,12 +176,12 @@ static int prepare_rhs(const Geo& g, const void* gauge, int prec, int recon, con
 
 // s_o = R^-1 eta_o + kappa R^-1 D_oe s_e   (all inside the full-lattice arrays, stride 2 pb)
 static int reconstruct_odd(const Geo& g, const void* gauge, int prec, int recon, void* s_full, const void* eta_full, double kappa,
-                           double mu, int nrhs, cudaStream_t st)
+                           double mu, int nrhs, cudaStream_t st, const void* link_cache = nullptr)
 {
     const size_t pb = spinor_parity_bytes(g, prec);
     const double a = 2.0 * kappa * mu, n = 1.0 / (1.0 + a * a);
     DslashParams p;
-    p.gauge = gauge; p.nrhs = nrhs; p.active = nullptr;
+    p.gauge = gauge; p.nrhs = nrhs; p.active = nullptr; p.link_cache = link_cache;
     p.out = static_cast<char*>(s_full) + pb; p.in = s_full; p.x = static_cast<const char*>(eta_full) + pb;
     p.out_parity = 1; p.dagger = 0;
     p.rhs_stride_out = p.rhs_stride_in = p.rhs_stride_x = 2 * pb;
@@ -188,9 +189,13 @@ static int reconstruct_odd(const Geo& g, const void* gauge, int prec, int recon,
     return launch_dslash(g, prec, recon, p, st);
 }
 
+// The multi-rhs tile kernel (more than 6 right-hand sides, fp32 / fp16 storage) stages its links from a per-solve cache:
+// one build (~0.3 ms at 32^3x64) serves the ~40-50 dslash launches of a truncated solve.
+static inline bool lp_uses_link_cache(int prec, int nrhs) { return prec != 8 && nrhs > 6; }
+
 size_t cg_lp_workspace_bytes(const Geo& g, int prec, int nrhs)
 {
-    return ctx_bytes(nrhs) + 6 * round256(spinor_parity_bytes(g, prec) * nrhs);
+    return ctx_bytes(nrhs) + 6 * round256(spinor_parity_bytes(g, prec) * nrhs) + (lp_uses_link_cache(prec, nrhs) ? link_cache_bytes(g, prec) : 0);
 }
 
 // truncated LP solve, batched
@@ -206,10 +211,12 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
     void* Ap = cv.take(pb * nrhs);
     void* t1 = cv.take(2 * pb * nrhs); // t1, t2 contiguous (mdagm_apply tmp)
     void* t2 = static_cast<char*>(t1) + pb * nrhs;
+    void* lc = lp_uses_link_cache(prec, nrhs) ? cv.take(link_cache_bytes(g, prec)) : nullptr;
     if (!cv.ok()) return TM_ERR_LAYOUT;
     int rc;
     if ((rc = init_ctx(c, prm, nrhs, st)) != TM_OK) return rc;
-    if ((rc = prepare_rhs(g, gauge, prec, recon, eta_full, b, t1, t2, prm->kappa, prm->mu, nrhs, st)) != TM_OK) return rc;
+    if (lc && (rc = link_cache_build(g, prec, recon, gauge, lc, st)) != TM_OK) return rc;
+    if ((rc = prepare_rhs(g, gauge, prec, recon, eta_full, b, t1, t2, prm->kappa, prm->mu, nrhs, st, lc)) != TM_OK) return rc;
     if ((rc = k_norm2<FIN_INIT>(g, prec, V_(b, pb), c, nrhs, st)) != TM_OK) return rc;
     if ((rc = k_convert(g, prec, prec, V_(r, pb), V_(p, pb), V_(b, pb), nrhs, st)) != TM_OK) return rc;
     VecArg x = V_(s_full, 2 * pb); // s_e lives in the even block of s_full
@@ -219,7 +226,7 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
     for (int k = 0; k < prm->max_iter;) {
         for (int j = 0; j < every && k < prm->max_iter; ++j, ++k)
             if ((rc = k_cg_iter(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), V_(Ap, pb), t1, prm->kappa, prm->mu, c, nrhs, true,
-                                st)) != TM_OK)
+                                st, lc)) != TM_OK)
                 return rc;
         TM_CUDA_CHECK(cudaMemcpyAsync(hact, c.active, nrhs, cudaMemcpyDeviceToHost, st));
         TM_CUDA_CHECK(cudaStreamSynchronize(st));
@@ -227,10 +234,10 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
         for (int q = 0; q < nrhs; ++q) any |= hact[q] != 0;
         if (!any) break;
     }
-    if ((rc = reconstruct_odd(g, gauge, prec, recon, s_full, eta_full, prm->kappa, prm->mu, nrhs, st)) != TM_OK) return rc;
+    if ((rc = reconstruct_odd(g, gauge, prec, recon, s_full, eta_full, prm->kappa, prm->mu, nrhs, st, lc)) != TM_OK) return rc;
     // recomputed residual of the normal system, in the same storage/arithmetic: Ap = A x; Ap = b - Ap
     if (!prm->skip_true_resid) {
-        if ((rc = mdagm_apply(g, gauge, prec, recon, Ap, pb, s_full, 2 * pb, t1, 0, prm->kappa, prm->mu, nrhs, nullptr, st)) != TM_OK) return rc;
+        if ((rc = mdagm_apply(g, gauge, prec, recon, Ap, pb, s_full, 2 * pb, t1, 0, prm->kappa, prm->mu, nrhs, nullptr, st, lc)) != TM_OK) return rc;
         if ((rc = k_axpby<1>(g, prec, prec, V_(Ap, pb), V_(b, pb), -1.0, 1.0, c, nrhs, st)) != TM_OK) return rc;
     }
     std::vector<CgScal> h(nrhs);

@@ -28,6 +28,7 @@ struct DslashKArgs {
     size_t link_block; // bytes of one (parity, mu) block
     size_t stride_out, stride_in, stride_x;
     const unsigned char* active;
+    const char* link_cache; // optional: tile images built by link_cache_kernel (tm_dslash_tile.cuh)
     int parity; // of the output sites
     int nrhs;
     double eps;  // +1, or -1 for the daggered operator

@@ -8,6 +8,9 @@
 
 namespace tmk {
 
+template <int PREC, int RECON>
+int link_cache_build_t(const Geo& g, const void* gauge, void* cache, cudaStream_t st);
+
 template <>
 int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cudaStream_t st)
 {
@@ -22,6 +25,7 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     a.stride_in = p.rhs_stride_in;
     a.stride_x = p.rhs_stride_x;
     a.active = p.active;
+    a.link_cache = static_cast<const char*>(p.link_cache);
     a.parity = p.out_parity;
     a.nrhs = p.nrhs;
     a.eps = p.dagger ? -1.0 : 1.0;
@@ -40,17 +44,24 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     const bool dg = p.dagger != 0;
     if (n == 1) {
         switch (cfg_single) {
-        case 0: launch_tile<TM_PREC, TM_RECON, 128, 1, 4, false, true>(a, dg, st); break;
-        case 1: launch_tile<TM_PREC, TM_RECON, 128, 1, 4, false, false>(a, dg, st); break;
-        case 2: launch_tile<TM_PREC, TM_RECON, 128, 1, 5, false, true>(a, dg, st); break;
+        case 0: launch_tile<TM_PREC, TM_RECON, 128, 1, 4, 0, true>(a, dg, st); break;
+        case 1: launch_tile<TM_PREC, TM_RECON, 128, 1, 4, 0, false>(a, dg, st); break;
+        case 2: launch_tile<TM_PREC, TM_RECON, 128, 1, 5, 0, true>(a, dg, st); break;
         default: launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
         }
     } else if (cfg_multi == 0) {
-        if (n <= 4) launch_tile<TM_PREC, TM_RECON, 32, 4, 6, true, false>(a, dg, st);
-        else if (n <= 6) launch_tile<TM_PREC, TM_RECON, 32, 6, 4, true, false>(a, dg, st);
-        else launch_tile<TM_PREC, TM_RECON, 32, 12, 2, true, false>(a, dg, st);
+        if (n <= 4) launch_tile<TM_PREC, TM_RECON, 32, 4, 6, 1, false>(a, dg, st);
+        else if (n <= 6) launch_tile<TM_PREC, TM_RECON, 32, 6, 4, 1, false>(a, dg, st);
+        else if (a.link_cache) {
+            static const int tpc = getenv("TM_DSLASH_TPC") ? atoi(getenv("TM_DSLASH_TPC")) : 4;
+            if (tpc == 1) launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 1>(a, dg, st);
+            else if (tpc == 2) launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 2>(a, dg, st);
+            else if (tpc == 8) launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 8>(a, dg, st);
+            else launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 4>(a, dg, st);
+        }
+        else launch_tile<TM_PREC, TM_RECON, 32, 12, 2, 1, false>(a, dg, st);
     } else if (cfg_multi == 1) {
-        launch_tile<TM_PREC, TM_RECON, 32, 12, 2, true, true>(a, dg, st);
+        launch_tile<TM_PREC, TM_RECON, 32, 12, 2, 1, true>(a, dg, st);
     } else {
         if (n % 3 == 0) launch_nr<TM_PREC, TM_RECON, 3>(a, n / 3, st);
         else if (n % 4 == 0) launch_nr<TM_PREC, TM_RECON, 4>(a, n / 4, st);
@@ -62,5 +73,19 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     TM_LAUNCH_CHECK("dslash_kernel");
     return TM_OK;
 }
+
+#if TM_PREC != 8
+template <>
+int link_cache_build_t<TM_PREC, TM_RECON>(const Geo& g, const void* gauge, void* cache, cudaStream_t st)
+{
+    DslashKArgs a = {};
+    a.g = g;
+    a.gauge = static_cast<const char*>(gauge);
+    a.link_block = link_block_bytes(g, TM_PREC, TM_RECON);
+    launch_link_cache<TM_PREC, TM_RECON>(a, static_cast<char*>(cache), st);
+    TM_LAUNCH_CHECK("link_cache_kernel");
+    return TM_OK;
+}
+#endif
 
 } // namespace tmk
