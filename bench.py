@@ -175,7 +175,7 @@ def run_b200(args, rank, world, local_rank):
     loops = torch.zeros((NRHS, 16, T, 2), dtype=torch.float64, device="cuda")
     tsm_ws = tm.device_buffer(tm.tm_tsm_workspace_bytes(L, prec, NRHS))
     loops_host = torch.zeros((NRHS, 16, T, 2), dtype=torch.float64).pin_memory()
-    prm = tm.make_cg_params(kappa, mu, LP_TOL, 500, tm.TM_CG_LP_TRUNCATED, 0.1, 4, 1)  # truncated mode: no residual recomputation
+    prm = tm.make_cg_params(kappa, mu, LP_TOL, 500, tm.TM_CG_LP_TRUNCATED, 0.1, 0, 1)  # truncated mode: no residual recomputation
     iters_log = []
 
     def step(i):

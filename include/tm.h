@@ -113,7 +113,9 @@ typedef struct {
     int max_iter;
     int mode;              /* tm_cg_mode */
     double reliable_delta; /* HP_MIXED: recompute the true residual in prec_hp when |r| drops by this factor (0 -> 0.1) */
-    int check_every;       /* host polls the device convergence flag every this many iterations (0 -> 4) */
+    int check_every;       /* LP_TRUNCATED: > 0: the host synchronises and reads the convergence flags every this many iterations;
+                              0: pipelined poll -- flags follow every iteration into pinned host memory, the host stays one
+                              iteration ahead of the GPU and stops one iteration after the last rhs converged */
     int skip_true_resid;   /* LP_TRUNCATED: 1 = do not recompute |b'' - A x| after the solve (saves one M^dag M);
                               info.true_resid is then -1.  The truncated mode never uses it. */
 } tm_cg_params;

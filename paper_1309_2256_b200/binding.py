@@ -205,7 +205,7 @@ def tm_cg_workspace_bytes(L, prec_hp, prec_lp, mode, nrhs=1):
     return load().tm_cg_workspace_bytes(L.handle, prec_hp, prec_lp, mode, nrhs)
 
 
-def make_cg_params(kappa, mu, tol, max_iter, mode, reliable_delta=0.1, check_every=4, skip_true_resid=0):
+def make_cg_params(kappa, mu, tol, max_iter, mode, reliable_delta=0.1, check_every=0, skip_true_resid=0):
     return tm_cg_params(kappa, mu, tol, max_iter, mode, reliable_delta, check_every, skip_true_resid)
 
 

@@ -212,7 +212,7 @@ namespace tmk {
 // M_pc^dag M_pc on `parity` with explicit strides/active flags (shared by tm_MdagM and the CG driver)
 int mdagm_apply(const Geo& g, const void* gauge, int prec, int recon, void* out, size_t out_stride, const void* in,
                 size_t in_stride, void* tmp, int parity, double kappa, double mu, int nrhs, const unsigned char* active,
-                cudaStream_t st, const void* link_cache)
+                cudaStream_t st, const void* link_cache, double* dot_partial)
 {
     const size_t pb = spinor_parity_bytes(g, prec);
     char* t1 = static_cast<char*>(tmp);
@@ -240,6 +240,11 @@ int mdagm_apply(const Geo& g, const void* gauge, int prec, int recon, void* out,
     p.out = out; p.in = t1; p.x = t2; p.out_parity = parity;
     p.rhs_stride_out = out_stride;
     kind_pq(TM_KIND_XPAY_TWIST, 1, kappa, mu, p.pq);
+    if (dot_partial) { // <in, M^dag M in> partials from the last launch's epilogue
+        p.dot_with = in;
+        p.dot_stride = in_stride;
+        p.dot_partial = dot_partial;
+    }
     return launch_dslash(g, prec, recon, p, st);
 }
 } // namespace tmk

@@ -25,7 +25,7 @@ struct CgScal {
     int iter;
     int max_iter;
     int status;     // tm_status
-    int pad;
+    int alpha_iter; // iteration (0-based) whose <p,Ap> produced `alpha`: update_xp applies x += alpha p only for that one
 };
 
 struct BlasCtx {
@@ -56,6 +56,45 @@ __device__ __forceinline__ double block_sum(double v)
     return s;
 }
 
+// what a finished reduction means for the per-rhs CG scalars (one thread)
+template <int FIN>
+__device__ __forceinline__ void finish_scalar(const BlasCtx& c, int rhs, double tot)
+{
+    CgScal& s = c.scal[rhs];
+    if (FIN == FIN_AUX) {
+        s.aux = tot;
+    } else if (FIN == FIN_INIT) { // tot = |b''|^2 : start of a solve
+        s.b2 = tot;
+        s.rr = tot;
+        if (!(tot > 0.0)) c.active[rhs] = 0; // zero source: x = 0 is the solution
+    } else if (FIN == FIN_PAP) {
+        s.pAp = tot;
+        s.alpha_iter = s.iter;
+        if (!(tot > 0.0)) { // breakdown or NaN
+            s.status = TM_ERR_BREAKDOWN;
+            s.alpha = 0.0;
+            c.active[rhs] = 0;
+        } else {
+            s.alpha = s.rr / tot;
+        }
+    } else { // FIN_RR: tot = |r_{k+1}|^2
+        s.rr_new = tot;
+        s.beta = tot / s.rr;
+        s.rr = tot;
+        s.iter += 1;
+        if (tot <= s.tol2 * s.b2) {
+            c.active[rhs] = 0;
+            s.status = TM_OK;
+        } else if (s.iter >= s.max_iter) {
+            c.active[rhs] = 0;
+            s.status = TM_ERR_MAXITER;
+        } else if (!(tot == tot)) {
+            c.active[rhs] = 0;
+            s.status = TM_ERR_BREAKDOWN;
+        }
+    }
+}
+
 // two-stage deterministic reduction + scalar update by the last block of this rhs
 template <int FIN>
 __device__ __forceinline__ void reduce_finalize(const BlasCtx& c, int rhs, double local)
@@ -77,38 +116,7 @@ __device__ __forceinline__ void reduce_finalize(const BlasCtx& c, int rhs, doubl
     for (int b = threadIdx.x; b < (int)gridDim.x; b += BLAS_THREADS) v += p[b];
     const double tot = block_sum(v);
     if (threadIdx.x == 0) {
-        CgScal& s = c.scal[rhs];
-        if (FIN == FIN_AUX) {
-            s.aux = tot;
-        } else if (FIN == FIN_INIT) { // tot = |b''|^2 : start of a solve
-            s.b2 = tot;
-            s.rr = tot;
-            if (!(tot > 0.0)) c.active[rhs] = 0; // zero source: x = 0 is the solution
-        } else if (FIN == FIN_PAP) {
-            s.pAp = tot;
-            if (!(tot > 0.0)) { // breakdown or NaN
-                s.status = TM_ERR_BREAKDOWN;
-                s.alpha = 0.0;
-                c.active[rhs] = 0;
-            } else {
-                s.alpha = s.rr / tot;
-            }
-        } else { // FIN_RR: tot = |r_{k+1}|^2
-            s.rr_new = tot;
-            s.beta = tot / s.rr;
-            s.rr = tot;
-            s.iter += 1;
-            if (tot <= s.tol2 * s.b2) {
-                c.active[rhs] = 0;
-                s.status = TM_OK;
-            } else if (s.iter >= s.max_iter) {
-                c.active[rhs] = 0;
-                s.status = TM_ERR_MAXITER;
-            } else if (!(tot == tot)) {
-                c.active[rhs] = 0;
-                s.status = TM_ERR_BREAKDOWN;
-            }
-        }
+        finish_scalar<FIN>(c, rhs, tot);
         c.tickets[rhs] = 0;
     }
 }
@@ -263,6 +271,74 @@ __global__ void __launch_bounds__(BLAS_THREADS) axpby_kernel(int Vh, VecArg y_, 
         acc += (double)s;
     }
     if (REDUCE) reduce_finalize<FIN_AUX>(c, rhs, acc);
+}
+
+// ---- fused truncated-CG iteration (LP mode): 8 vector passes per iteration instead of 11 --------------------------
+//   <p,Ap> partials come out of the last dslash of M^dag M (warp_dot_store, tm_dslash.cuh); dot_finalize_kernel sums them in
+//   a fixed order -> alpha;  update_r: r -= alpha Ap, |r|^2 -> beta, convergence;  update_xp: x += alpha p, p = r + beta p.
+
+// pAp[rhs] = sum_g partial[rhs][g] (fixed order), then the FIN_PAP scalar update.  grid = nrhs blocks
+__global__ void __launch_bounds__(BLAS_THREADS) dot_finalize_kernel(const double* partial, int ngroups, BlasCtx c)
+{
+    const int rhs = blockIdx.x;
+    if (!c.active[rhs]) return;
+    double v = 0.0;
+    const double* p = partial + (size_t)rhs * ngroups;
+    for (int g = threadIdx.x; g < ngroups; g += BLAS_THREADS) v += p[g];
+    const double tot = block_sum(v);
+    if (threadIdx.x == 0) finish_scalar<FIN_PAP>(c, rhs, tot);
+}
+
+// r -= alpha Ap; rr_new = |r|^2; beta, convergence
+template <int PREC>
+__global__ void __launch_bounds__(BLAS_THREADS) update_r_kernel(int Vh, VecArg r_, VecArg Ap_, BlasCtx c)
+{
+    typedef typename Prec<PREC>::real real;
+    const int rhs = blockIdx.y;
+    if (!c.active[rhs]) return;
+    const real alpha = (real)c.scal[rhs].alpha;
+    double acc = 0.0;
+    for (int cb = blockIdx.x * BLAS_THREADS + threadIdx.x; cb < Vh; cb += gridDim.x * BLAS_THREADS) {
+        real r[24], q[24];
+        load_spinor<PREC>(r_.p + rhs * r_.stride, Vh, cb, r);
+        load_spinor<PREC>(Ap_.p + rhs * Ap_.stride, Vh, cb, q);
+        real s = 0;
+#pragma unroll
+        for (int k = 0; k < 24; ++k) {
+            r[k] = fma(-alpha, q[k], r[k]);
+            s = fma(r[k], r[k], s);
+        }
+        store_spinor<PREC>(r_.p + rhs * r_.stride, Vh, cb, r);
+        acc += (double)s;
+    }
+    reduce_finalize<FIN_RR>(c, rhs, acc);
+}
+
+// iteration `iter` (0-based): x += alpha p for every rhs whose alpha belongs to this iteration (also the one that has just
+// converged); p = r + beta p for the rhs that are still active
+template <int PREC>
+__global__ void __launch_bounds__(BLAS_THREADS) update_xp_kernel(int Vh, VecArg x_, VecArg p_, VecArg r_, BlasCtx c, int iter)
+{
+    typedef typename Prec<PREC>::real real;
+    const int rhs = blockIdx.y;
+    if (c.scal[rhs].alpha_iter != iter || c.scal[rhs].alpha == 0.0) return;
+    const bool more = c.active[rhs] != 0;
+    const real alpha = (real)c.scal[rhs].alpha, beta = (real)c.scal[rhs].beta;
+    for (int cb = blockIdx.x * BLAS_THREADS + threadIdx.x; cb < Vh; cb += gridDim.x * BLAS_THREADS) {
+        real x[24], p[24];
+        load_spinor<PREC>(x_.p + rhs * x_.stride, Vh, cb, x);
+        load_spinor<PREC>(p_.p + rhs * p_.stride, Vh, cb, p);
+#pragma unroll
+        for (int k = 0; k < 24; ++k) x[k] = fma(alpha, p[k], x[k]);
+        store_spinor<PREC>(x_.p + rhs * x_.stride, Vh, cb, x);
+        if (more) {
+            real r[24];
+            load_spinor<PREC>(r_.p + rhs * r_.stride, Vh, cb, r);
+#pragma unroll
+            for (int k = 0; k < 24; ++k) p[k] = fma(beta, p[k], r[k]);
+            store_spinor<PREC>(p_.p + rhs * p_.stride, Vh, cb, p);
+        }
+    }
 }
 
 static inline int blas_blocks(int Vh)

@@ -90,6 +90,27 @@ static int k_cg_iter(const Geo& g, const void* gauge, int prec, int recon, VecAr
     });
 }
 
+// one truncated-CG iteration with the reductions fused into the operator (LP mode): 4 dslash + 3 vector kernels, 8 passes
+static int k_cg_iter_fused(const Geo& g, const void* gauge, int prec, int recon, VecArg x, VecArg r, VecArg p, VecArg Ap, void* tmp,
+                           double kappa, double mu, const BlasCtx& c, double* dot_partial, int nrhs, int iter, cudaStream_t st,
+                           const void* link_cache)
+{
+    int rc = mdagm_apply(g, gauge, prec, recon, Ap.p, Ap.stride, p.p, p.stride, tmp, 0, kappa, mu, nrhs, c.active, st, link_cache,
+                         dot_partial);
+    if (rc != TM_OK) return rc;
+    dim3 grid(blas_blocks(g.Vh), nrhs);
+    return by_prec(prec, [&](auto P) {
+        constexpr int PR = decltype(P)::value;
+        dot_finalize_kernel<<<nrhs, BLAS_THREADS, 0, st>>>(dot_partial, (g.Vh + 31) / 32, c);
+        TM_LAUNCH_CHECK("dot_finalize_kernel");
+        update_r_kernel<PR><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, r, Ap, c);
+        TM_LAUNCH_CHECK("update_r_kernel");
+        update_xp_kernel<PR><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, x, p, r, c, iter);
+        TM_LAUNCH_CHECK("update_xp_kernel");
+        return (int)TM_OK;
+    });
+}
+
 static int k_update_p(const Geo& g, int prec, VecArg p, VecArg r, const BlasCtx& c, int nrhs, cudaStream_t st)
 {
     dim3 grid(blas_blocks(g.Vh), nrhs);
@@ -98,6 +119,26 @@ static int k_update_p(const Geo& g, int prec, VecArg p, VecArg r, const BlasCtx&
         TM_LAUNCH_CHECK("update_p_kernel");
         return (int)TM_OK;
     });
+}
+
+// pinned host ring for the pipelined convergence poll of cg_lp_truncated (library-owned host memory, created once)
+struct PollRing {
+    static constexpr int DEPTH = 4;
+    unsigned char* flags = nullptr; // [DEPTH][TM_MAX_NRHS], pinned
+    cudaEvent_t ev[DEPTH];
+};
+static PollRing* poll_ring()
+{
+    static thread_local PollRing ring;
+    static thread_local bool ok = false;
+    if (!ok) {
+        if (cudaHostAlloc(reinterpret_cast<void**>(&ring.flags), PollRing::DEPTH * TM_MAX_NRHS, cudaHostAllocDefault) != cudaSuccess)
+            return nullptr;
+        for (int i = 0; i < PollRing::DEPTH; ++i)
+            if (cudaEventCreateWithFlags(&ring.ev[i], cudaEventDisableTiming) != cudaSuccess) return nullptr;
+        ok = true;
+    }
+    return &ring;
 }
 
 // carve a workspace
@@ -138,6 +179,7 @@ static int init_ctx(const BlasCtx& c, const tm_cg_params* p, int nrhs, cudaStrea
         s.tol2 = p->tol * p->tol;
         s.max_iter = p->max_iter;
         s.status = TM_ERR_MAXITER;
+        s.alpha_iter = -1;
     }
     TM_CUDA_CHECK(cudaMemcpyAsync(c.scal, h.data(), sizeof(CgScal) * nrhs, cudaMemcpyHostToDevice, st));
     TM_CUDA_CHECK(cudaMemsetAsync(c.active, 1, nrhs, st));
@@ -192,10 +234,11 @@ static int reconstruct_odd(const Geo& g, const void* gauge, int prec, int recon,
 // The multi-rhs tile kernel (more than 6 right-hand sides, fp32 / fp16 storage) stages its links from a per-solve cache:
 // one build (~0.3 ms at 32^3x64) serves the ~40-50 dslash launches of a truncated solve.
 static inline bool lp_uses_link_cache(int prec, int nrhs) { return prec != 8 && nrhs > 6; }
+static inline size_t dot_partial_bytes(const Geo& g, int nrhs) { return round256(sizeof(double) * (size_t)((g.Vh + 31) / 32) * nrhs); }
 
 size_t cg_lp_workspace_bytes(const Geo& g, int prec, int nrhs)
 {
-    return ctx_bytes(nrhs) + 6 * round256(spinor_parity_bytes(g, prec) * nrhs) + (lp_uses_link_cache(prec, nrhs) ? link_cache_bytes(g, prec) : 0);
+    return ctx_bytes(nrhs) + dot_partial_bytes(g, nrhs) + 6 * round256(spinor_parity_bytes(g, prec) * nrhs) + (lp_uses_link_cache(prec, nrhs) ? link_cache_bytes(g, prec) : 0);
 }
 
 // truncated LP solve, batched
@@ -212,6 +255,7 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
     void* t1 = cv.take(2 * pb * nrhs); // t1, t2 contiguous (mdagm_apply tmp)
     void* t2 = static_cast<char*>(t1) + pb * nrhs;
     void* lc = lp_uses_link_cache(prec, nrhs) ? cv.take(link_cache_bytes(g, prec)) : nullptr;
+    double* dotp = static_cast<double*>(cv.take(dot_partial_bytes(g, nrhs)));
     if (!cv.ok()) return TM_ERR_LAYOUT;
     int rc;
     if ((rc = init_ctx(c, prm, nrhs, st)) != TM_OK) return rc;
@@ -221,18 +265,42 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
     if ((rc = k_convert(g, prec, prec, V_(r, pb), V_(p, pb), V_(b, pb), nrhs, st)) != TM_OK) return rc;
     VecArg x = V_(s_full, 2 * pb); // s_e lives in the even block of s_full
     TM_CUDA_CHECK(cudaMemset2DAsync(s_full, 2 * pb, 0, pb, nrhs, st));
-    const int every = prm->check_every > 0 ? prm->check_every : 4;
-    unsigned char hact[TM_MAX_NRHS];
-    for (int k = 0; k < prm->max_iter;) {
-        for (int j = 0; j < every && k < prm->max_iter; ++j, ++k)
-            if ((rc = k_cg_iter(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), V_(Ap, pb), t1, prm->kappa, prm->mu, c, nrhs, true,
-                                st, lc)) != TM_OK)
+    if (prm->check_every > 0) {
+        // poll the device flags every `check_every` iterations (one stream synchronisation per poll)
+        const int every = prm->check_every;
+        unsigned char hact[TM_MAX_NRHS];
+        for (int k = 0; k < prm->max_iter;) {
+            for (int j = 0; j < every && k < prm->max_iter; ++j, ++k)
+                if ((rc = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), V_(Ap, pb), t1, prm->kappa, prm->mu, c, dotp,
+                                          nrhs, k, st, lc)) != TM_OK)
+                    return rc;
+            TM_CUDA_CHECK(cudaMemcpyAsync(hact, c.active, nrhs, cudaMemcpyDeviceToHost, st));
+            TM_CUDA_CHECK(cudaStreamSynchronize(st));
+            bool any = false;
+            for (int q = 0; q < nrhs; ++q) any |= hact[q] != 0;
+            if (!any) break;
+        }
+    } else {
+        // pipelined polling (check_every = 0): the flags of every iteration go to pinned host memory behind an event; the host
+        // keeps one iteration queued ahead of the GPU and stops one iteration after the last right-hand side converged (the
+        // extra iteration's kernels find no active rhs and exit).  The device never waits for the host.
+        PollRing* ring = poll_ring();
+        if (!ring) return TM_ERR_CUDA;
+        for (int k = 0; k < prm->max_iter; ++k) {
+            if ((rc = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), V_(Ap, pb), t1, prm->kappa, prm->mu, c, dotp, nrhs,
+                                      k, st, lc)) != TM_OK)
                 return rc;
-        TM_CUDA_CHECK(cudaMemcpyAsync(hact, c.active, nrhs, cudaMemcpyDeviceToHost, st));
-        TM_CUDA_CHECK(cudaStreamSynchronize(st));
-        bool any = false;
-        for (int q = 0; q < nrhs; ++q) any |= hact[q] != 0;
-        if (!any) break;
+            const int slot = k % PollRing::DEPTH;
+            TM_CUDA_CHECK(cudaMemcpyAsync(ring->flags + slot * TM_MAX_NRHS, c.active, nrhs, cudaMemcpyDeviceToHost, st));
+            TM_CUDA_CHECK(cudaEventRecord(ring->ev[slot], st));
+            if (k >= 1) { // look at iteration k-1 while iteration k runs
+                const int prev = (k - 1) % PollRing::DEPTH;
+                TM_CUDA_CHECK(cudaEventSynchronize(ring->ev[prev]));
+                bool any = false;
+                for (int q = 0; q < nrhs; ++q) any |= ring->flags[prev * TM_MAX_NRHS + q] != 0;
+                if (!any) break;
+            }
+        }
     }
     if ((rc = reconstruct_odd(g, gauge, prec, recon, s_full, eta_full, prm->kappa, prm->mu, nrhs, st, lc)) != TM_OK) return rc;
     // recomputed residual of the normal system, in the same storage/arithmetic: Ap = A x; Ap = b - Ap

@@ -85,6 +85,10 @@ struct DslashParams {
     size_t rhs_stride_out, rhs_stride_in, rhs_stride_x; // bytes between consecutive right-hand sides
     const unsigned char* active; // optional per-rhs device flags: rhs with active[r] == 0 is skipped (may be null)
     const void* link_cache = nullptr; // optional: link_cache_build() output for this gauge field (fp32 / fp16, nrhs > 6)
+    // optional fused reduction: dot_partial[rhs][ceil(Vh/32)] = per-warp sums of Re <dot_with, out>
+    const void* dot_with = nullptr;
+    size_t dot_stride = 0;
+    double* dot_partial = nullptr;
 };
 int launch_dslash(const Geo& g, int prec, int recon, const DslashParams& p, cudaStream_t st);
 void kind_pq(int kind, int dagger, double kappa, double mu, double pq[4]);
@@ -93,7 +97,7 @@ size_t link_cache_bytes(const Geo& g, int prec);
 int link_cache_build(const Geo& g, int prec, int recon, const void* gauge, void* cache, cudaStream_t st);
 int mdagm_apply(const Geo& g, const void* gauge, int prec, int recon, void* out, size_t out_stride, const void* in,
                 size_t in_stride, void* tmp, int parity, double kappa, double mu, int nrhs, const unsigned char* active,
-                cudaStream_t st, const void* link_cache = nullptr);
+                cudaStream_t st, const void* link_cache = nullptr, double* dot_partial = nullptr);
 int spinor_pack_any(const Geo& g, long long V, int prec, int mode, const double* src, double* dst, const unsigned char* codes,
                     void* packed, int nrhs, cudaStream_t st);
 int loop_contract(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,

@@ -29,6 +29,9 @@ struct DslashKArgs {
     size_t stride_out, stride_in, stride_x;
     const unsigned char* active;
     const char* link_cache; // optional: tile images built by link_cache_kernel (tm_dslash_tile.cuh)
+    const char* dot_with;   // optional fused reduction: dot_partial[rhs][cb / 32] = sum over the warp of Re <dot_with, out>
+    size_t stride_dot;
+    double* dot_partial;
     int parity; // of the output sites
     int nrhs;
     double eps;  // +1, or -1 for the daggered operator
@@ -127,6 +130,30 @@ __device__ __forceinline__ void su3_mul(const real* u, const real* h, real* g)
             g[6 * s + 2 * a] = re;
             g[6 * s + 2 * a + 1] = im;
         }
+}
+
+// Fused CG reduction: Re <w, out> of one site in the arithmetic precision, summed over the warp's 32
+// consecutive sites in fp64 with a fixed shuffle tree; lane 0 stores the partial of site group cb / 32.  `o` is the
+// epilogue result before storage rounding.  Every lane of the warp that reaches the epilogue calls this (the active
+// lanes are the contiguous range [0, n) because cb grows with the lane).
+template <int PREC>
+__device__ __forceinline__ void warp_dot_store(const DslashKArgs& a, int rhs, int cb, const typename Prec<PREC>::real* o)
+{
+    typedef typename Prec<PREC>::real real;
+    real w[24];
+    load_spinor<PREC>(a.dot_with + (size_t)rhs * a.stride_dot, a.g.Vh, cb, w);
+    real s = 0;
+#pragma unroll
+    for (int k = 0; k < 24; ++k) s = fma(w[k], o[k], s);
+    double v = (double)s;
+    const unsigned m = __activemask();
+    const int n = __popc(m), lane = threadIdx.x & 31;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const double t = __shfl_down_sync(m, v, off);
+        if (lane + off < n) v += t;
+    }
+    if (lane == 0) a.dot_partial[(size_t)rhs * ((a.g.Vh + 31) >> 5) + (cb >> 5)] = v;
 }
 
 template <int PREC, int RECON, int NR, int MU, int FWD>
@@ -231,6 +258,7 @@ __global__ void __launch_bounds__(256) dslash_kernel(const DslashKArgs a)
             }
         }
         store_spinor<PREC>(a.out + (size_t)(r0 + r) * a.stride_out, Vh, cb, o);
+        if (a.dot_partial != nullptr) warp_dot_store<PREC>(a, r0 + r, cb, o);
     }
 }
 

@@ -299,6 +299,7 @@ __device__ __forceinline__ void tile_site(const DslashKArgs& a, const SM& sm, in
         }
     }
     store_spinor<PREC>(a.out + (size_t)rhs * a.stride_out, Vh, cb, o);
+    if (a.dot_partial != nullptr) warp_dot_store<PREC>(a, rhs, cb, o);
 }
 
 // phase A for one tile: neighbour indices (the antiperiodic sign of a temporal hop rides on the index as ~index) and the
