@@ -230,7 +230,10 @@ int mdagm_apply(const Geo& g, const void* gauge, int prec, int recon, void* out,
     p.out = t2; p.in = t1; p.x = in; p.out_parity = parity;
     p.rhs_stride_in = pb; p.rhs_stride_x = in_stride;
     kind_pq(TM_KIND_XPAY_TWIST, 0, kappa, mu, p.pq);
+    // <in, M_pc^dag M_pc in> = |M_pc in|^2: the CG's <p,Ap> falls out of this launch's epilogue with no extra load
+    p.dot_partial = dot_partial;
     if ((rc = launch_dslash(g, prec, recon, p, st)) != TM_OK) return rc;
+    p.dot_partial = nullptr;
     // t1 = R(-a)^-1 D^dag_{pbar p} t2
     p.out = t1; p.in = t2; p.x = nullptr; p.out_parity = 1 - parity; p.dagger = 1;
     p.rhs_stride_x = pb;
@@ -240,11 +243,6 @@ int mdagm_apply(const Geo& g, const void* gauge, int prec, int recon, void* out,
     p.out = out; p.in = t1; p.x = t2; p.out_parity = parity;
     p.rhs_stride_out = out_stride;
     kind_pq(TM_KIND_XPAY_TWIST, 1, kappa, mu, p.pq);
-    if (dot_partial) { // <in, M^dag M in> partials from the last launch's epilogue
-        p.dot_with = in;
-        p.dot_stride = in_stride;
-        p.dot_partial = dot_partial;
-    }
     return launch_dslash(g, prec, recon, p, st);
 }
 } // namespace tmk

@@ -85,7 +85,7 @@ struct DslashParams {
     size_t rhs_stride_out, rhs_stride_in, rhs_stride_x; // bytes between consecutive right-hand sides
     const unsigned char* active; // optional per-rhs device flags: rhs with active[r] == 0 is skipped (may be null)
     const void* link_cache = nullptr; // optional: link_cache_build() output for this gauge field (fp32 / fp16, nrhs > 6)
-    // optional fused reduction: dot_partial[rhs][ceil(Vh/32)] = per-warp sums of Re <dot_with, out>
+    // optional fused reduction: dot_partial[rhs][ceil(Vh/32)] = per-warp sums of Re <dot_with, out> (|out|^2 if dot_with is null)
     const void* dot_with = nullptr;
     size_t dot_stride = 0;
     double* dot_partial = nullptr;

@@ -29,7 +29,8 @@ struct DslashKArgs {
     size_t stride_out, stride_in, stride_x;
     const unsigned char* active;
     const char* link_cache; // optional: tile images built by link_cache_kernel (tm_dslash_tile.cuh)
-    const char* dot_with;   // optional fused reduction: dot_partial[rhs][cb / 32] = sum over the warp of Re <dot_with, out>
+    const char* dot_with;   // optional fused reduction: dot_partial[rhs][cb / 32] = sum over the warp of Re <dot_with, out>,
+                            // or of |out|^2 if dot_with is null
     size_t stride_dot;
     double* dot_partial;
     int parity; // of the output sites
@@ -132,7 +133,7 @@ __device__ __forceinline__ void su3_mul(const real* u, const real* h, real* g)
         }
 }
 
-// Fused CG reduction: Re <w, out> of one site in the arithmetic precision, summed over the warp's 32
+// Fused CG reduction: Re <w, out> (or |out|^2 when there is no w) of one site in the arithmetic precision, summed over the warp's 32
 // consecutive sites in fp64 with a fixed shuffle tree; lane 0 stores the partial of site group cb / 32.  `o` is the
 // epilogue result before storage rounding.  Every lane of the warp that reaches the epilogue calls this (the active
 // lanes are the contiguous range [0, n) because cb grows with the lane).
@@ -140,11 +141,16 @@ template <int PREC>
 __device__ __forceinline__ void warp_dot_store(const DslashKArgs& a, int rhs, int cb, const typename Prec<PREC>::real* o)
 {
     typedef typename Prec<PREC>::real real;
-    real w[24];
-    load_spinor<PREC>(a.dot_with + (size_t)rhs * a.stride_dot, a.g.Vh, cb, w);
     real s = 0;
+    if (a.dot_with != nullptr) {
+        real w[24];
+        load_spinor<PREC>(a.dot_with + (size_t)rhs * a.stride_dot, a.g.Vh, cb, w);
 #pragma unroll
-    for (int k = 0; k < 24; ++k) s = fma(w[k], o[k], s);
+        for (int k = 0; k < 24; ++k) s = fma(w[k], o[k], s);
+    } else { // |out|^2
+#pragma unroll
+        for (int k = 0; k < 24; ++k) s = fma(o[k], o[k], s);
+    }
     double v = (double)s;
     const unsigned m = __activemask();
     const int n = __popc(m), lane = threadIdx.x & 31;

@@ -28,7 +28,7 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     a.link_cache = static_cast<const char*>(p.link_cache);
     a.dot_with = static_cast<const char*>(p.dot_with);
     a.stride_dot = p.dot_stride;
-    a.dot_partial = p.dot_with ? p.dot_partial : nullptr;
+    a.dot_partial = p.dot_partial;
     a.parity = p.out_parity;
     a.nrhs = p.nrhs;
     a.eps = p.dagger ? -1.0 : 1.0;
