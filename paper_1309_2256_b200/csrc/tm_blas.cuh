@@ -273,11 +273,13 @@ __global__ void __launch_bounds__(BLAS_THREADS) axpby_kernel(int Vh, VecArg y_, 
     if (REDUCE) reduce_finalize<FIN_AUX>(c, rhs, acc);
 }
 
-// ---- fused truncated-CG iteration (LP mode): 8 vector passes per iteration instead of 11 --------------------------
-//   <p,Ap> partials come out of the last dslash of M^dag M (warp_dot_store, tm_dslash.cuh); dot_finalize_kernel sums them in
-//   a fixed order -> alpha;  update_r: r -= alpha Ap, |r|^2 -> beta, convergence;  update_xp: x += alpha p, p = r + beta p.
+// ---- fused truncated-CG iteration (LP mode) ------------------------------------------------------------------------
+//   <p,Ap> = |M_pc p|^2 and |r|^2 come out of dslash epilogues as per-warp partials (warp_dot_store, tm_dslash.cuh), the
+//   residual update r -= alpha A p happens in the epilogue that produces A p (fused_axpy); dot_finalize_kernel sums the
+//   partials in a fixed order -> alpha / beta, convergence;  update_xp: x += alpha p, p = r + beta p (5 vector passes).
 
-// pAp[rhs] = sum_g partial[rhs][g] (fixed order), then the FIN_PAP scalar update.  grid = nrhs blocks
+// tot[rhs] = sum_g partial[rhs][g] (fixed order), then the FIN scalar update (FIN_PAP or FIN_RR).  grid = nrhs blocks
+template <int FIN>
 __global__ void __launch_bounds__(BLAS_THREADS) dot_finalize_kernel(const double* partial, int ngroups, BlasCtx c)
 {
     const int rhs = blockIdx.x;
@@ -286,32 +288,7 @@ __global__ void __launch_bounds__(BLAS_THREADS) dot_finalize_kernel(const double
     const double* p = partial + (size_t)rhs * ngroups;
     for (int g = threadIdx.x; g < ngroups; g += BLAS_THREADS) v += p[g];
     const double tot = block_sum(v);
-    if (threadIdx.x == 0) finish_scalar<FIN_PAP>(c, rhs, tot);
-}
-
-// r -= alpha Ap; rr_new = |r|^2; beta, convergence
-template <int PREC>
-__global__ void __launch_bounds__(BLAS_THREADS) update_r_kernel(int Vh, VecArg r_, VecArg Ap_, BlasCtx c)
-{
-    typedef typename Prec<PREC>::real real;
-    const int rhs = blockIdx.y;
-    if (!c.active[rhs]) return;
-    const real alpha = (real)c.scal[rhs].alpha;
-    double acc = 0.0;
-    for (int cb = blockIdx.x * BLAS_THREADS + threadIdx.x; cb < Vh; cb += gridDim.x * BLAS_THREADS) {
-        real r[24], q[24];
-        load_spinor<PREC>(r_.p + rhs * r_.stride, Vh, cb, r);
-        load_spinor<PREC>(Ap_.p + rhs * Ap_.stride, Vh, cb, q);
-        real s = 0;
-#pragma unroll
-        for (int k = 0; k < 24; ++k) {
-            r[k] = fma(-alpha, q[k], r[k]);
-            s = fma(r[k], r[k], s);
-        }
-        store_spinor<PREC>(r_.p + rhs * r_.stride, Vh, cb, r);
-        acc += (double)s;
-    }
-    reduce_finalize<FIN_RR>(c, rhs, acc);
+    if (threadIdx.x == 0) finish_scalar<FIN>(c, rhs, tot);
 }
 
 // iteration `iter` (0-based): x += alpha p for every rhs whose alpha belongs to this iteration (also the one that has just

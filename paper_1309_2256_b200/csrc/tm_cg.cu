@@ -90,22 +90,46 @@ static int k_cg_iter(const Geo& g, const void* gauge, int prec, int recon, VecAr
     });
 }
 
-// one truncated-CG iteration with the reductions fused into the operator (LP mode): 4 dslash + 3 vector kernels, 8 passes
-static int k_cg_iter_fused(const Geo& g, const void* gauge, int prec, int recon, VecArg x, VecArg r, VecArg p, VecArg Ap, void* tmp,
-                           double kappa, double mu, const BlasCtx& c, double* dot_partial, int nrhs, int iter, cudaStream_t st,
-                           const void* link_cache)
+// One truncated-CG iteration (LP mode) with the reductions and the residual update fused into the operator:
+//   t1 = R^-1 D p;  t2 = M_pc p, partials of |t2|^2 = <p, A p>;  [finalize -> alpha]
+//   t1 = R(-a)^-1 D^dag t2;  r = r - alpha (R(-a) t2 - kappa^2 D^dag t1), partials of |r|^2;  [finalize -> beta, convergence]
+//   x += alpha p, p = r + beta p.
+// A p is never written to memory; the only vector kernel left moves 5 one-parity spinors per rhs (11 before).
+static int k_cg_iter_fused(const Geo& g, const void* gauge, int prec, int recon, VecArg x, VecArg r, VecArg p, void* tmp, double kappa,
+                           double mu, const BlasCtx& c, double* partial, int nrhs, int iter, cudaStream_t st, const void* link_cache)
 {
-    int rc = mdagm_apply(g, gauge, prec, recon, Ap.p, Ap.stride, p.p, p.stride, tmp, 0, kappa, mu, nrhs, c.active, st, link_cache,
-                         dot_partial);
-    if (rc != TM_OK) return rc;
+    const size_t pb = spinor_parity_bytes(g, prec);
+    char* t1 = static_cast<char*>(tmp);
+    char* t2 = t1 + pb * nrhs;
+    const int ngroups = (g.Vh + 31) / 32;
+    DslashParams d;
+    d.gauge = gauge; d.nrhs = nrhs; d.active = c.active; d.link_cache = link_cache;
+    d.rhs_stride_out = d.rhs_stride_in = d.rhs_stride_x = pb;
+    int rc;
+    d.out = t1; d.in = p.p; d.x = nullptr; d.out_parity = 1; d.dagger = 0; d.rhs_stride_in = p.stride;
+    kind_pq(TM_KIND_TWIST_INV, 0, kappa, mu, d.pq);
+    if ((rc = launch_dslash(g, prec, recon, d, st)) != TM_OK) return rc;
+    d.out = t2; d.in = t1; d.x = p.p; d.out_parity = 0; d.rhs_stride_in = pb; d.rhs_stride_x = p.stride;
+    kind_pq(TM_KIND_XPAY_TWIST, 0, kappa, mu, d.pq);
+    d.dot_partial = partial;
+    if ((rc = launch_dslash(g, prec, recon, d, st)) != TM_OK) return rc;
+    d.dot_partial = nullptr;
+    dot_finalize_kernel<FIN_PAP><<<nrhs, BLAS_THREADS, 0, st>>>(partial, ngroups, c);
+    TM_LAUNCH_CHECK("dot_finalize_kernel");
+    d.out = t1; d.in = t2; d.x = nullptr; d.out_parity = 1; d.dagger = 1; d.rhs_stride_x = pb;
+    kind_pq(TM_KIND_TWIST_INV, 1, kappa, mu, d.pq);
+    if ((rc = launch_dslash(g, prec, recon, d, st)) != TM_OK) return rc;
+    d.out = r.p; d.in = t1; d.x = t2; d.out_parity = 0; d.rhs_stride_out = r.stride;
+    kind_pq(TM_KIND_XPAY_TWIST, 1, kappa, mu, d.pq);
+    d.axpy_y = r.p; d.axpy_y_stride = r.stride;
+    d.axpy_coef = &c.scal[0].alpha; d.axpy_coef_stride = sizeof(CgScal);
+    d.dot_partial = partial;
+    if ((rc = launch_dslash(g, prec, recon, d, st)) != TM_OK) return rc;
+    dot_finalize_kernel<FIN_RR><<<nrhs, BLAS_THREADS, 0, st>>>(partial, ngroups, c);
+    TM_LAUNCH_CHECK("dot_finalize_kernel");
     dim3 grid(blas_blocks(g.Vh), nrhs);
     return by_prec(prec, [&](auto P) {
-        constexpr int PR = decltype(P)::value;
-        dot_finalize_kernel<<<nrhs, BLAS_THREADS, 0, st>>>(dot_partial, (g.Vh + 31) / 32, c);
-        TM_LAUNCH_CHECK("dot_finalize_kernel");
-        update_r_kernel<PR><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, r, Ap, c);
-        TM_LAUNCH_CHECK("update_r_kernel");
-        update_xp_kernel<PR><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, x, p, r, c, iter);
+        update_xp_kernel<decltype(P)::value><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, x, p, r, c, iter);
         TM_LAUNCH_CHECK("update_xp_kernel");
         return (int)TM_OK;
     });
@@ -271,8 +295,8 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
         unsigned char hact[TM_MAX_NRHS];
         for (int k = 0; k < prm->max_iter;) {
             for (int j = 0; j < every && k < prm->max_iter; ++j, ++k)
-                if ((rc = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), V_(Ap, pb), t1, prm->kappa, prm->mu, c, dotp,
-                                          nrhs, k, st, lc)) != TM_OK)
+                if ((rc = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), t1, prm->kappa, prm->mu, c, dotp, nrhs, k,
+                                          st, lc)) != TM_OK)
                     return rc;
             TM_CUDA_CHECK(cudaMemcpyAsync(hact, c.active, nrhs, cudaMemcpyDeviceToHost, st));
             TM_CUDA_CHECK(cudaStreamSynchronize(st));
@@ -287,8 +311,8 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
         PollRing* ring = poll_ring();
         if (!ring) return TM_ERR_CUDA;
         for (int k = 0; k < prm->max_iter; ++k) {
-            if ((rc = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), V_(Ap, pb), t1, prm->kappa, prm->mu, c, dotp, nrhs,
-                                      k, st, lc)) != TM_OK)
+            if ((rc = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), t1, prm->kappa, prm->mu, c, dotp, nrhs, k, st,
+                                      lc)) != TM_OK)
                 return rc;
             const int slot = k % PollRing::DEPTH;
             TM_CUDA_CHECK(cudaMemcpyAsync(ring->flags + slot * TM_MAX_NRHS, c.active, nrhs, cudaMemcpyDeviceToHost, st));

@@ -89,6 +89,11 @@ struct DslashParams {
     const void* dot_with = nullptr;
     size_t dot_stride = 0;
     double* dot_partial = nullptr;
+    // optional fused axpy: out = axpy_y - coef[rhs] * (epilogue result), coef = device doubles at axpy_coef + rhs * axpy_coef_stride
+    const void* axpy_y = nullptr;
+    size_t axpy_y_stride = 0;
+    const void* axpy_coef = nullptr;
+    size_t axpy_coef_stride = 0;
 };
 int launch_dslash(const Geo& g, int prec, int recon, const DslashParams& p, cudaStream_t st);
 void kind_pq(int kind, int dagger, double kappa, double mu, double pq[4]);

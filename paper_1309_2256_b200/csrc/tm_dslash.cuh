@@ -33,6 +33,11 @@ struct DslashKArgs {
                             // or of |out|^2 if dot_with is null
     size_t stride_dot;
     double* dot_partial;
+    // optional fused axpy: out = y - coef[rhs] * (epilogue result); coef is a device double per rhs (byte stride stride_coef)
+    const char* axpy_y;
+    size_t stride_y;
+    const char* axpy_coef;
+    size_t stride_coef;
     int parity; // of the output sites
     int nrhs;
     double eps;  // +1, or -1 for the daggered operator
@@ -131,6 +136,18 @@ __device__ __forceinline__ void su3_mul(const real* u, const real* h, real* g)
             g[6 * s + 2 * a] = re;
             g[6 * s + 2 * a + 1] = im;
         }
+}
+
+// out = y - coef[rhs] * o  (the CG residual update r -= alpha A p done in the epilogue that produces A p)
+template <int PREC>
+__device__ __forceinline__ void fused_axpy(const DslashKArgs& a, int rhs, int cb, typename Prec<PREC>::real* o)
+{
+    typedef typename Prec<PREC>::real real;
+    real y[24];
+    load_spinor<PREC>(a.axpy_y + (size_t)rhs * a.stride_y, a.g.Vh, cb, y);
+    const real c = (real)(*reinterpret_cast<const double*>(a.axpy_coef + (size_t)rhs * a.stride_coef));
+#pragma unroll
+    for (int k = 0; k < 24; ++k) o[k] = fma(-c, o[k], y[k]);
 }
 
 // Fused CG reduction: Re <w, out> (or |out|^2 when there is no w) of one site in the arithmetic precision, summed over the warp's 32
@@ -263,6 +280,7 @@ __global__ void __launch_bounds__(256) dslash_kernel(const DslashKArgs a)
                 o[2 * k + 1] += p0 * xv[2 * k + 1] + s5 * p1 * xv[2 * k];
             }
         }
+        if (a.axpy_y != nullptr) fused_axpy<PREC>(a, r0 + r, cb, o);
         store_spinor<PREC>(a.out + (size_t)(r0 + r) * a.stride_out, Vh, cb, o);
         if (a.dot_partial != nullptr) warp_dot_store<PREC>(a, r0 + r, cb, o);
     }

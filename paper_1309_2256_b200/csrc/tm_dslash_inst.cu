@@ -29,6 +29,10 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     a.dot_with = static_cast<const char*>(p.dot_with);
     a.stride_dot = p.dot_stride;
     a.dot_partial = p.dot_partial;
+    a.axpy_y = static_cast<const char*>(p.axpy_y);
+    a.stride_y = p.axpy_y_stride;
+    a.axpy_coef = static_cast<const char*>(p.axpy_coef);
+    a.stride_coef = p.axpy_coef_stride;
     a.parity = p.out_parity;
     a.nrhs = p.nrhs;
     a.eps = p.dagger ? -1.0 : 1.0;

@@ -298,6 +298,7 @@ __device__ __forceinline__ void tile_site(const DslashKArgs& a, const SM& sm, in
             o[2 * k + 1] += p0 * xv[2 * k + 1] + s5 * p1 * xv[2 * k];
         }
     }
+    if (a.axpy_y != nullptr) fused_axpy<PREC>(a, rhs, cb, o);
     store_spinor<PREC>(a.out + (size_t)rhs * a.stride_out, Vh, cb, o);
     if (a.dot_partial != nullptr) warp_dot_store<PREC>(a, rhs, cb, o);
 }
