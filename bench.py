@@ -33,7 +33,7 @@ FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12          # 148 SMs x 128 FP32 
 
 
 # one `ncu --set full` capture of the dominant kernel (profiles/r01_ncu_dslash_fp16_recon12_12rhs.md), bytes per launch
-NCU_DRAM_BYTES_PER_LAUNCH = 1.9256e9
+NCU_DRAM_BYTES_PER_LAUNCH = 2.6016e9
 
 
 def peaks():
@@ -241,14 +241,15 @@ def run_b200(args, rank, world, local_rank):
         tot_flops += Vh * NRHS * (3 * FLOPS_XPAY + 1 * FLOPS_TWIST_INV)
         for k in range(1, max(it) + 1):
             act = sum(1 for x in it if x >= k)
-            tot_bytes += 4 * Vh * 8 * recon * prec + Vh * act * (4 * 2 + 2) * sp
-            tot_flops += Vh * act * 2 * (FLOPS_TWIST_INV + FLOPS_XPAY)
+            # 4 launches: in + out each, x twice, the residual once; flops: 2 x (TWIST_INV + XPAY) + |M p|^2, r -= alpha A p, |r|^2
+            tot_bytes += 4 * Vh * 8 * recon * prec + Vh * act * (4 * 2 + 3) * sp
+            tot_flops += Vh * act * (2 * (FLOPS_TWIST_INV + FLOPS_XPAY) + 3 * 48)
     k_avg_ms = k_ms / max(1, k_n)
     ach_gbs = tot_bytes / (k_ms * 1e-3) / 1e9
     ach_tf = tot_flops / (k_ms * 1e-3) / 1e12
-    roofline = {"kernel": "dslash_tile_kernel<fp16,recon12,32 sites x 12 rhs per CTA>", "bound": "alu", "achieved": ach_tf, "peak": FP32_PEAK_TFLOPS,
+    roofline = {"kernel": "dslash_tile_lc_kernel<fp16,recon12,12 rhs per CTA,4 tiles per CTA> (link cache + cp.async.bulk)", "bound": "alu", "achieved": ach_tf, "peak": FP32_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": ach_tf / FP32_PEAK_TFLOPS, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
-                "traffic_source": "profiles/r01_ncu_dslash_fp16_recon12_12rhs.md: dram__bytes_read.sum + dram__bytes_write.sum, mean of 4 launches (2 TWIST_INV + 2 XPAY_TWIST, 12 active rhs); algorithmic mean 1.837e9",
+                "traffic_source": "profiles/r01_ncu_dslash_fp16_recon12_12rhs.md: dram__bytes_read.sum + dram__bytes_write.sum, mean of 4 launches (2 TWIST_INV, XPAY_TWIST + norm, XPAY_TWIST^dag + residual update; 12 active rhs, link cache); algorithmic mean 2.437e9",
                 "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks)",
                 "avg_launch_ms": k_avg_ms, "launches_timed": int(k_n), "share_of_step": k_ms / (ms_step * args.steps),
                 "hbm_view": {"achieved_GBps": ach_gbs, "peak_GBps": hbm_peak, "frac": ach_gbs / hbm_peak, "peak_source": peak_src}}
