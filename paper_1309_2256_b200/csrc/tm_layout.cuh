@@ -123,8 +123,9 @@ __device__ __forceinline__ void rebuild_row2(real* u)
         const int j1 = (j + 1) % 3, j2 = (j + 2) % 3;
         const real ar = u[2 * j1], ai = u[2 * j1 + 1], br = u[6 + 2 * j2], bi = u[6 + 2 * j2 + 1];
         const real cr = u[2 * j2], ci = u[2 * j2 + 1], dr = u[6 + 2 * j1], di = u[6 + 2 * j1 + 1];
-        u[12 + 2 * j] = (ar * br - ai * bi) - (cr * dr - ci * di);
-        u[12 + 2 * j + 1] = -((ar * bi + ai * br) - (cr * di + ci * dr));
+        // one multiply + three FMAs per real (8 instead of 10 operations per complex entry)
+        u[12 + 2 * j] = fma(ci, di, fma(-cr, dr, fma(-ai, bi, ar * br)));
+        u[12 + 2 * j + 1] = fma(ci, dr, fma(cr, di, fma(-ai, br, -(ar * bi))));
     }
 }
 
