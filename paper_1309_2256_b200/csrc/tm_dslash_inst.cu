@@ -44,10 +44,10 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     else launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
 #else
     // Launch shapes from the B200 sweep; the environment knobs exist for re-tuning:
-    //   TM_DSLASH_SINGLE: 0 = 128 registers + prefetch, 1 = 128 registers, 2 = 96 registers + prefetch, -1 = dslash_kernel
+    //   TM_DSLASH_SINGLE: 0 = 128 registers + prefetch, 1 = 128 registers (default), 2 = 96 registers + prefetch, -1 = dslash_kernel
     //   TM_DSLASH_MULTI : 0 = by nrhs (12 / 6 / 4 right-hand sides per CTA at 80 registers), 1 = 12 + prefetch, -1 = dslash_kernel
     static const int cfg_multi = getenv("TM_DSLASH_MULTI") ? atoi(getenv("TM_DSLASH_MULTI")) : 0;
-    static const int cfg_single = getenv("TM_DSLASH_SINGLE") ? atoi(getenv("TM_DSLASH_SINGLE")) : (TM_PREC == 2 ? 2 : 1);
+    static const int cfg_single = getenv("TM_DSLASH_SINGLE") ? atoi(getenv("TM_DSLASH_SINGLE")) : 1;
     const bool dg = p.dagger != 0;
     if (n == 1) {
         switch (cfg_single) {
