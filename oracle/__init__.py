@@ -194,3 +194,48 @@ def tsm_combine(L_hp, L_lp_same, L_lp):
             l = l + L_lp[j]
         out = out + l / len(L_lp)
     return out
+
+
+# ---- NEXT-2 / NEXT-3: plain numpy definitions in oracle/insertions.py ---------------------------
+from . import insertions as _ins  # noqa: E402
+
+covdev = _ins.covdev
+contract_field = _ins.contract_field
+momenta_p2_max = _ins.momenta_p2_max
+time_dilute = _ins.time_dilute
+
+
+def _Gammas():
+    return np.array([Gamma(n) for n in range(16)])
+
+
+def loop_momentum(a, b, momenta):
+    """L[n][t][k] = sum_xvec exp(-i p_k xvec) a^dag Gamma_n b; momenta int [K][3]."""
+    return _ins.loop_momentum(a, b, momenta, _Gammas())
+
+
+def loop_derivative(U, a, b, mu, ap=True):
+    """One-derivative insertion: L[n][t] = sum_x a(x)^dag Gamma_n (D_mu b)(x)."""
+    return loop(a, covdev(U, b, mu, ap=ap))
+
+
+def loop_slice(a, b, t0):
+    """Single-time-slice contraction, complex [16]."""
+    return _ins.loop_slice(_c(a), _c(b), t0, _Gammas())
+
+
+def hpe_remainder(U, s, kappa, mu, ap=True):
+    """(B H)^4 s of PAPER.md:160 Eq. (16)/(17): B = R(2 kappa mu)^-1, H = -kappa Dslash."""
+    a = 2 * kappa * mu
+    return _ins.hpe_remainder(lambda v: hop(U, v, ap=ap), lambda v: twist(v, a, inverse=True), _c(s), kappa)
+
+
+def hpe_series(U, eta, kappa, mu, ap=True):
+    """B eta - B H B eta + (BH)^2 B eta - (BH)^3 B eta (first four terms of Eq. 16)."""
+    a = 2 * kappa * mu
+    return _ins.hpe_series(lambda v: hop(U, v, ap=ap), lambda v: twist(v, a, inverse=True), _c(eta), kappa)
+
+
+def hpe_local_traces(kappa, mu):
+    """Per-site Tr[Gamma_n (B - BHB + (BH)^2 B - (BH)^3 B)]_xx, complex [16] (gauge independent)."""
+    return _ins.hpe_local_traces(kappa, mu, np.array([gamma(m) for m in range(5)]), _Gammas())
