@@ -181,6 +181,51 @@ int tm_oneend_loops(const tm_lattice* L, const void* gauge, int prec, int recon,
 int tm_tsm_combine(int T, const double* loops_hp, const double* loops_lp_same, int n_hp, const double* loops_lp, int n_lp,
                    double* out, void* stream);
 
+/* ---- NEXT-2: the paper's contraction kernels in full (App. A.2) ------------------ */
+/* "A covariant-derivative kernel was also developed to allow the calculation of one-derivative insertions".
+ * out = D_mu in on the full lattice, D_mu psi(x) = 1/2 [s U_mu(x) psi(x+mu) - s U_mu(x-mu)^dag psi(x-mu)] (central difference,
+ * DESIGN.md reading 27; s = antiperiodic sign of a temporal hop; spin untouched).  mu = 0..3 = x,y,z,t.
+ * in_full / out_full: DEVICE packed full-lattice spinors [nrhs][parity][...], must not alias.  One-derivative loops are
+ * tm_loop_contract(a, D_mu b). */
+int tm_covdev(const tm_lattice* L, const void* gauge, int prec, int recon, void* out_full, const void* in_full, int mu, int nrhs,
+              void* stream);
+
+/* Colour-traced contraction with the Dirac and volume indices open:
+ *   out[rhs][site][al][be] = sum_c conj(a_{al c}(site)) b_{be c}(site), site = x + X (y + Y (z + Z t)).
+ * out: DEVICE double [nrhs][V][4][4][2] (the layout an FFT over the volume index takes).  Products in the
+ * storage arithmetic (fp32 for fp32/fp16 fields), stored as fp64. */
+int tm_contract_field(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* stream);
+
+/* Momentum-projected loops (PAPER.md:421 "data is sent ... for FFT ... we usually insert here a cut-off in p^2", :427 p^2 <= 9):
+ *   out[rhs][n][t][k] = sum_{xvec} exp(-i p_k . xvec) a(x)^dag Gamma_n b(x),  p_k = 2 pi (m_x/X, m_y/Y, m_z/Z)
+ * (forward-DFT sign, reading 28).  The contraction is fused with a separable partial DFT for the listed momenta;
+ * the contraction field never goes to memory.  momenta: HOST int [n_momenta][3] = (m_x, m_y, m_z), |m_i| <= 4 (else
+ * TM_ERR_ARG); copied to the device inside the call.  out: DEVICE double [nrhs][16][T][n_momenta][2].
+ * workspace: DEVICE, tm_loop_momentum_workspace_bytes(L, nrhs, n_momenta, pmax) with pmax >= max |m_i|.
+ * Fixed summation order, fp64 accumulation. */
+size_t tm_loop_momentum_workspace_bytes(const tm_lattice* L, int nrhs, int n_momenta, int pmax);
+int tm_loop_momentum(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, const int* momenta,
+                     int n_momenta, double* out, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- NEXT-3: time dilution and hopping-parameter expansion ---------------------------------------- */
+/* Time dilution / coherent sources: out = in on the time slices with keep_slice[t] != 0, zero elsewhere.
+ * keep_slice: HOST uint8 [T] (T <= 512).  in_full / out_full: DEVICE packed full-lattice [nrhs][parity][...]; may alias. */
+int tm_time_dilute(const tm_lattice* L, const void* in_full, int prec, int nrhs, const unsigned char* keep_slice, void* out_full,
+                   void* stream);
+/* Single-time-slice contraction: out[rhs][n] = sum_{x: x4 = t0} a(x)^dag Gamma_n b(x); reads slice t0 only.
+ * out: DEVICE double [nrhs][16][2]; workspace as tm_loop_contract. */
+int tm_loop_contract_slice(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, int t0, double* out,
+                           void* workspace, void* stream);
+/* HPE, Eq. (16): M_u^-1 = B - BHB + (BH)^2 B - (BH)^3 B + (BH)^4 M_u^-1, B = (1 + i 2 kappa mu g5)^-1,
+ * H = 2 kappa D = -kappa Dslash (reading 2).  out = (B H)^4 s: contracted with the source it estimates the
+ * stochastic fifth term (Eq. 17).  8 fused dslash launches.  tmp_full: DEVICE scratch of the size of s_full; no aliasing. */
+int tm_hpe_remainder(const tm_lattice* L, const void* gauge, int prec, int recon, void* out_full, const void* s_full, void* tmp_full,
+                     double kappa, double mu, int nrhs, void* stream);
+/* The exact terms of Eq. (16) for an ultra-local insertion, per site: out16[n] = Tr_{spin,colour}[Gamma_n (B - BHB + (BH)^2 B
+ * - (BH)^3 B)]_{xx} = 3 tr[Gamma_n (B + kappa^2 sum_mu (B(1-g_mu)B(1+g_mu)B + B(1+g_mu)B(1-g_mu)B))]; gauge independent, odd
+ * powers vanish.  Multiply by X Y Z for a time slice.  out16: HOST double [16][2].  Host arithmetic only. */
+int tm_hpe_local_traces(double kappa, double mu, double* out16);
+
 /* ---- end-to-end TSM batch with HOST buffers ("the source is sent to the GPUs for inversion and
  *      contraction, and contractions are stored back in the CPUs") ----------------------------------------- */
 /* codes_host: HOST (pinned recommended) uint8 [nrhs][V][12] Z2xiZ2 codes; loops_host: HOST double [nrhs][16][T][2].

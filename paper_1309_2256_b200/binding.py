@@ -22,7 +22,8 @@ ABI_SYMBOLS = [
     "tm_dslash_general", "tm_MdagM", "tm_cg_workspace_bytes", "tm_cg_multi", "tm_cg", "tm_loop_workspace_bytes",
     "tm_loop_contract", "tm_loop_contract_ex", "tm_M", "tm_oneend_workspace_bytes", "tm_oneend_loops", "tm_tsm_combine",
     "tm_tsm_workspace_bytes", "tm_tsm_batch_host", "tm_launch_count", "tm_kernel_timing_enable",
-    "tm_kernel_timing_read",
+    "tm_kernel_timing_read", "tm_covdev", "tm_contract_field", "tm_loop_momentum_workspace_bytes", "tm_loop_momentum",
+    "tm_time_dilute", "tm_loop_contract_slice", "tm_hpe_remainder", "tm_hpe_local_traces",
 ]
 
 
@@ -89,6 +90,14 @@ def load():
         "tm_launch_count": (ctypes.c_ulonglong, []),
         "tm_kernel_timing_enable": (i, [i]),
         "tm_kernel_timing_read": (i, [P(d), P(ctypes.c_longlong), i]),
+        "tm_covdev": (i, [vp, vp, i, i, vp, vp, i, i, vp]),
+        "tm_contract_field": (i, [vp, vp, vp, i, i, vp, vp]),
+        "tm_loop_momentum_workspace_bytes": (sz, [vp, i, i, i]),
+        "tm_loop_momentum": (i, [vp, vp, vp, i, i, P(i), i, vp, vp, sz, vp]),
+        "tm_time_dilute": (i, [vp, vp, i, i, ctypes.c_char_p, vp, vp]),
+        "tm_loop_contract_slice": (i, [vp, vp, vp, i, i, i, vp, vp, vp]),
+        "tm_hpe_remainder": (i, [vp, vp, i, i, vp, vp, vp, d, d, i, vp]),
+        "tm_hpe_local_traces": (i, [d, d, P(d)]),
     }
     for name, (res, args) in sig.items():
         f = getattr(lib, name)
@@ -273,6 +282,52 @@ def tm_tsm_batch_host(L, gauge_lp, prec_lp, recon, codes_host, params, nrhs, loo
                                   _ptr(loops_host), _ptr(workspace), ws_bytes, _stream(stream))
     _check(rc, "tm_tsm_batch_host", allow=_SOFT)
     return rc, list(info)
+
+
+def tm_covdev(L, gauge, prec, recon, out_full, in_full, mu, nrhs=1, stream=None):
+    return _check(load().tm_covdev(L.handle, _ptr(gauge), prec, recon, _ptr(out_full), _ptr(in_full), mu, nrhs, _stream(stream)),
+                  "tm_covdev")
+
+
+def tm_contract_field(L, a_full, b_full, prec, nrhs, out, stream=None):
+    return _check(load().tm_contract_field(L.handle, _ptr(a_full), _ptr(b_full), prec, nrhs, _ptr(out), _stream(stream)),
+                  "tm_contract_field")
+
+
+def tm_loop_momentum_workspace_bytes(L, nrhs, n_momenta, pmax):
+    return load().tm_loop_momentum_workspace_bytes(L.handle, nrhs, n_momenta, pmax)
+
+
+def tm_loop_momentum(L, a_full, b_full, prec, nrhs, momenta, out, workspace, stream=None):
+    """momenta: host int array [K][3]."""
+    m = np.ascontiguousarray(momenta, dtype=np.int32)
+    ws_bytes = workspace.numel() * workspace.element_size()
+    return _check(load().tm_loop_momentum(L.handle, _ptr(a_full), _ptr(b_full), prec, nrhs,
+                                          m.ctypes.data_as(ctypes.POINTER(ctypes.c_int)), int(m.shape[0]), _ptr(out), _ptr(workspace),
+                                          ws_bytes, _stream(stream)), "tm_loop_momentum")
+
+
+def tm_time_dilute(L, in_full, prec, nrhs, keep_slice, out_full, stream=None):
+    """keep_slice: host sequence of T flags."""
+    k = bytes(bytearray(1 if v else 0 for v in keep_slice))
+    return _check(load().tm_time_dilute(L.handle, _ptr(in_full), prec, nrhs, k, _ptr(out_full), _stream(stream)), "tm_time_dilute")
+
+
+def tm_loop_contract_slice(L, a_full, b_full, prec, nrhs, t0, out, workspace, stream=None):
+    return _check(load().tm_loop_contract_slice(L.handle, _ptr(a_full), _ptr(b_full), prec, nrhs, int(t0), _ptr(out), _ptr(workspace),
+                                                _stream(stream)), "tm_loop_contract_slice")
+
+
+def tm_hpe_remainder(L, gauge, prec, recon, out_full, s_full, tmp_full, kappa, mu, nrhs=1, stream=None):
+    return _check(load().tm_hpe_remainder(L.handle, _ptr(gauge), prec, recon, _ptr(out_full), _ptr(s_full), _ptr(tmp_full), kappa, mu,
+                                          nrhs, _stream(stream)), "tm_hpe_remainder")
+
+
+def tm_hpe_local_traces(kappa, mu):
+    """Per-site exact HPE terms, complex [16] (host arithmetic in the library)."""
+    out = (ctypes.c_double * 32)()
+    _check(load().tm_hpe_local_traces(kappa, mu, out), "tm_hpe_local_traces")
+    return np.array(out[:]).view(np.complex128)
 
 
 def tm_launch_count():

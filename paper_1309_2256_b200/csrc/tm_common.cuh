@@ -110,6 +110,8 @@ int loop_contract(const Geo& g, const void* a_full, const void* b_full, int prec
 int loop_contract_ex(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,
                      int g5_left, int g5_right, double scale_re, double scale_im, cudaStream_t st);
 size_t loop_workspace_bytes(const Geo& g, int nrhs);
+int loop_contract_range(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,
+                        int g5_left, int g5_right, double scale_re, double scale_im, int t0, int nt, cudaStream_t st);
 void kernel_timing_begin(cudaStream_t st);
 void kernel_timing_end(cudaStream_t st);
 

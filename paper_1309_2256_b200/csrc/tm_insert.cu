@@ -1,0 +1,471 @@
+// tm_insert.cu -- SURVEY.md 8(f) NEXT-2 / NEXT-3: what the paper's contraction kernels and variance-reduction drivers add
+// to the hot path (PAPER.md:407-415 App. A.2 "Contraction kernels", :148-169 time-dilution and HPE, :421-427 FFT + p^2 cut).
+//
+//   tm_covdev            (D_mu psi)(x) = 1/2 [s U_mu(x) psi(x+mu) - s U_mu(x-mu)^dag psi(x-mu)]   "covariant-derivative kernel"
+//   tm_contract_field    C[x][al][be] = sum_c conj(a_{al c}(x)) b_{be c}(x)                        colour traced, Dirac + volume open
+//   tm_loop_momentum     L[n][t][k] = sum_xvec exp(-i p_k xvec) a^dag Gamma_n b                     contraction fused with a separable
+//                        partial DFT (x, then y, then z) for the few momenta kept (p^2 <= 9), instead of the paper's
+//                        field -> cuFFT -> cut: the 256 B/site field never goes to HBM
+//   tm_time_dilute       noise restricted to chosen time slices (time dilution, coherent sources)
+//   tm_hpe_remainder     (B H)^4 s, B = R^-1, H = -kappa Dslash: the stochastic term of Eq. (17)
+//   tm_hpe_local_traces  per-site Tr[Gamma_n (B - BHB + (BH)^2 B - (BH)^3 B)]_xx, the exact terms of Eq. (16) for ultra-local X
+// (tm_loop_contract_slice, the single-time-slice contraction, lives in tm_loop.cu.)
+#include "tm_dslash_tile.cuh"
+#include "tm_gamma.cuh"
+
+namespace tmk {
+
+// ---- covariant derivative ----------------------------------------------------------------------------------------
+// One thread per site of one parity; spin is untouched, so the two SU(3) products act on all four spin components.
+template <int PREC, int RECON>
+__global__ void __launch_bounds__(128) covdev_kernel(Geo g, const char* gauge, size_t link_block, char* out_full, const char* in_full,
+                                                     size_t parity_bytes, int mu)
+{
+    typedef typename Prec<PREC>::real real;
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    const int parity = blockIdx.y, rhs = blockIdx.z;
+    if (cb >= g.Vh) return;
+    int nb[8];
+    float sgp, sgm;
+    tile_neighbours(g, parity, cb, nb, sgp, sgm);
+    const int nf = nb[2 * mu], nbk = nb[2 * mu + 1];
+    const real sf = (mu == 3) ? (real)sgp : real(1), sb = (mu == 3) ? (real)sgm : real(1);
+    const char* in = in_full + (size_t)rhs * 2 * parity_bytes + (size_t)(1 - parity) * parity_bytes;
+    real u[18], v[24], gf[24], gb[24];
+    load_link<PREC, RECON>(gauge + (size_t)(parity * 4 + mu) * link_block, g.Vh, cb, u);
+    load_spinor<PREC>(in, g.Vh, nf, v);
+    su3_mul<0>(u, v, gf);
+    su3_mul<0>(u, v + 12, gf + 12);
+    load_link<PREC, RECON>(gauge + (size_t)((1 - parity) * 4 + mu) * link_block, g.Vh, nbk, u);
+    load_spinor<PREC>(in, g.Vh, nbk, v);
+    su3_mul<1>(u, v, gb);
+    su3_mul<1>(u, v + 12, gb + 12);
+    real o[24];
+    const real hf = real(0.5) * sf, hb = real(0.5) * sb;
+#pragma unroll
+    for (int k = 0; k < 24; ++k) o[k] = hf * gf[k] - hb * gb[k];
+    store_spinor<PREC>(out_full + (size_t)rhs * 2 * parity_bytes + (size_t)parity * parity_bytes, g.Vh, cb, o);
+}
+
+template <int PREC, int RECON>
+static int covdev_launch(const Geo& g, const void* gauge, void* out_full, const void* in_full, int mu, int nrhs, cudaStream_t st)
+{
+    dim3 grid((g.Vh + 127) / 128, 2, nrhs);
+    covdev_kernel<PREC, RECON><<<grid, 128, 0, st>>>(g, (const char*)gauge, link_block_bytes(g, PREC, RECON), (char*)out_full,
+                                                     (const char*)in_full, spinor_parity_bytes(g, PREC), mu);
+    TM_LAUNCH_CHECK("covdev_kernel");
+    return TM_OK;
+}
+
+// ---- contraction field -------------------------------------------------------------------------------------------
+// C_{al be}(x) of one site in the storage arithmetic (fp32 for fp32 / fp16 fields), as in loop_partial_kernel
+template <typename real>
+__device__ __forceinline__ void site_contract(const real* a, const real* b, real* c32)
+{
+#pragma unroll
+    for (int al = 0; al < 4; ++al)
+#pragma unroll
+        for (int be = 0; be < 4; ++be) {
+            real re = 0, im = 0;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const real ar = a[(al * 3 + c) * 2], ai = a[(al * 3 + c) * 2 + 1];
+                const real br = b[(be * 3 + c) * 2], bi = b[(be * 3 + c) * 2 + 1];
+                re = fma(ar, br, re);
+                re = fma(ai, bi, re);
+                im = fma(ar, bi, im);
+                im = fma(-ai, br, im);
+            }
+            c32[(al * 4 + be) * 2] = re;
+            c32[(al * 4 + be) * 2 + 1] = im;
+        }
+}
+
+// out[rhs][site][4][4][2] fp64, site lexicographic (x fastest) = 2 cb + (x odd): "fits exactly in the input required" by an
+// FFT.  Each warp transposes its 32 x 32 doubles through shared memory so that the stores are coalesced.
+template <int PREC>
+__global__ void __launch_bounds__(128) contract_field_kernel(Geo g, const char* a_full, const char* b_full, size_t parity_bytes,
+                                                             double* out, long long V)
+{
+    typedef typename Prec<PREC>::real real;
+    __shared__ double tile[4][32][33];
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    const int parity = blockIdx.y, rhs = blockIdx.z;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const bool valid = cb < g.Vh;
+    if (valid) {
+        real a[24], b[24], c[32];
+        load_spinor<PREC>(a_full + (size_t)rhs * 2 * parity_bytes + (size_t)parity * parity_bytes, g.Vh, cb, a);
+        load_spinor<PREC>(b_full + (size_t)rhs * 2 * parity_bytes + (size_t)parity * parity_bytes, g.Vh, cb, b);
+        site_contract<real>(a, b, c);
+#pragma unroll
+        for (int k = 0; k < 32; ++k) tile[warp][lane][k] = (double)c[k];
+    }
+    __syncwarp();
+    const int cb0 = cb - lane;
+    for (int s = 0; s < 32; ++s) {
+        const int c2 = cb0 + s;
+        if (c2 >= g.Vh) break;
+        uint32_t row, xh, rem2, y, t, z;
+        g.dXh.divmod((uint32_t)c2, row, xh);
+        g.dY.divmod(row, rem2, y);
+        g.dZ.divmod(rem2, t, z);
+        const size_t site = 2 * (size_t)c2 + ((parity + y + z + t) & 1);
+        out[((size_t)rhs * V + site) * 32 + lane] = tile[warp][s][lane];
+    }
+}
+
+} // namespace tmk
+
+namespace tmk {
+
+// ---- momentum-projected loops --------------------------------------------------------------------------------------
+// Stage 1 (one CTA per (z, t) plane and rhs): contraction of every site of the plane, DFT over x for the NP = 2 P + 1
+// values n_x = -P..P, then over y, accumulated per thread in fp64 in a fixed order:
+//     W2[rhs][t][z][ipx][ipy][ab] = sum_y e^{-2 pi i n_y y / Y} sum_x e^{-2 pi i n_x x / X} C_ab(x, y, z, t).
+// Stage 2 (loop_mom_final_kernel): DFT over z for the listed momenta and the 16 Gamma_n.
+constexpr int MOM_THREADS = 256;
+constexpr int MOM_ROWS = 4;   // y rows contracted per pass
+constexpr int MOM_MAXP = 4;   // |n_i| <= 4 (p^2 <= 9 needs 3)
+constexpr int MOM_ACC = (2 * MOM_MAXP + 1) * (2 * MOM_MAXP + 1) * 16 / MOM_THREADS + 1;
+
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ double2 cfma(double2 a, double2 b, double2 c)
+{
+    return make_double2(fma(a.x, b.x, fma(-a.y, b.y, c.x)), fma(a.x, b.y, fma(a.y, b.x, c.y)));
+}
+// exp(-2 pi i n k / N) with the argument reduced in integers first
+__device__ __forceinline__ double2 dft_phase(int n, int k, int N)
+{
+    int m = (n * k) % N;
+    if (m < 0) m += N;
+    double s, c;
+    sincospi(-2.0 * (double)m / (double)N, &s, &c);
+    return make_double2(c, s);
+}
+
+template <int PREC>
+__global__ void __launch_bounds__(MOM_THREADS) loop_mom_plane_kernel(Geo g, const char* a_full, const char* b_full,
+                                                                     size_t parity_bytes, int P, double2* W2)
+{
+    typedef typename Prec<PREC>::real real;
+    extern __shared__ double2 smem[];
+    const int X = g.X, Y = g.Y, NP = 2 * P + 1;
+    double2* ex = smem;                      // [NP][X]
+    double2* ey = ex + NP * X;               // [NP][Y]
+    double2* Cs = ey + NP * Y;               // [MOM_ROWS][X][16]
+    double2* W1 = Cs + MOM_ROWS * X * 16;    // [MOM_ROWS][NP][16]
+    const int z = blockIdx.x, t = blockIdx.y, rhs = blockIdx.z, tid = threadIdx.x;
+    for (int i = tid; i < NP * X; i += MOM_THREADS) ex[i] = dft_phase(i / X - P, i % X, X);
+    for (int i = tid; i < NP * Y; i += MOM_THREADS) ey[i] = dft_phase(i / Y - P, i % Y, Y);
+    double2 acc[MOM_ACC];
+#pragma unroll
+    for (int j = 0; j < MOM_ACC; ++j) acc[j] = make_double2(0.0, 0.0);
+    const int nout = NP * NP * 16;
+    const char* af = a_full + (size_t)rhs * 2 * parity_bytes;
+    const char* bf = b_full + (size_t)rhs * 2 * parity_bytes;
+    __syncthreads();
+    for (int y0 = 0; y0 < Y; y0 += MOM_ROWS) {
+        const int nr = min(MOM_ROWS, Y - y0);
+        // (1) contraction of the sites of rows y0 .. y0 + nr - 1
+        for (int i = tid; i < nr * X; i += MOM_THREADS) {
+            const int r = i / X, x = i - r * X, y = y0 + r;
+            const int parity = (x + y + z + t) & 1;
+            const int cb = (x >> 1) + g.Xh * (y + Y * (z + g.Z * t));
+            real a[24], b[24], c[32];
+            load_spinor<PREC>(af + (size_t)parity * parity_bytes, g.Vh, cb, a);
+            load_spinor<PREC>(bf + (size_t)parity * parity_bytes, g.Vh, cb, b);
+            site_contract<real>(a, b, c);
+#pragma unroll
+            for (int k = 0; k < 16; ++k) Cs[(r * X + x) * 16 + k] = make_double2((double)c[2 * k], (double)c[2 * k + 1]);
+        }
+        __syncthreads();
+        // (2) DFT over x
+        for (int o = tid; o < nr * NP * 16; o += MOM_THREADS) {
+            const int ab = o & 15, ip = (o >> 4) % NP, r = (o >> 4) / NP;
+            double2 s = make_double2(0.0, 0.0);
+            for (int x = 0; x < X; ++x) s = cfma(Cs[(r * X + x) * 16 + ab], ex[ip * X + x], s);
+            W1[(r * NP + ip) * 16 + ab] = s;
+        }
+        __syncthreads();
+        // (3) DFT over y, accumulated
+#pragma unroll
+        for (int j = 0; j < MOM_ACC; ++j) {
+            const int o = tid + j * MOM_THREADS;
+            if (o < nout) {
+                const int ab = o & 15, ipy = (o >> 4) % NP, ipx = (o >> 4) / NP;
+                for (int r = 0; r < nr; ++r) acc[j] = cfma(W1[(r * NP + ipx) * 16 + ab], ey[ipy * Y + y0 + r], acc[j]);
+            }
+        }
+        __syncthreads();
+    }
+    double2* dst = W2 + (((size_t)rhs * g.T + t) * g.Z + z) * nout;
+#pragma unroll
+    for (int j = 0; j < MOM_ACC; ++j) {
+        const int o = tid + j * MOM_THREADS;
+        if (o < nout) dst[o] = acc[j];
+    }
+}
+
+// out[rhs][n][t][k] = sum_ab (Gamma_n)_ab sum_z e^{-2 pi i n_z z / Z} W2[rhs][t][z][ipx_k][ipy_k][ab]
+__global__ void __launch_bounds__(128) loop_mom_final_kernel(Geo g, int P, const double2* W2, const int* mom, int K, GammaTable tb,
+                                                             double* out)
+{
+    __shared__ double2 Ck[8][16];
+    const int t = blockIdx.x, rhs = blockIdx.y;
+    const int NP = 2 * P + 1, nout = NP * NP * 16;
+    const int kk = threadIdx.x >> 4, ab = threadIdx.x & 15;
+    for (int k0 = 0; k0 < K; k0 += 8) {
+        const int k = k0 + kk;
+        if (k < K) {
+            const int nx = mom[3 * k], ny = mom[3 * k + 1], nz = mom[3 * k + 2];
+            const double2* src = W2 + ((size_t)rhs * g.T + t) * g.Z * nout + ((nx + P) * NP + (ny + P)) * 16 + ab;
+            double2 s = make_double2(0.0, 0.0);
+            for (int z = 0; z < g.Z; ++z) s = cfma(src[(size_t)z * nout], dft_phase(nz, z, g.Z), s);
+            Ck[kk][ab] = s;
+        }
+        __syncthreads();
+        if (k < K) {
+            const int n = ab;
+            double re = 0.0, im = 0.0;
+#pragma unroll
+            for (int al = 0; al < 4; ++al) {
+                const int be = tb.col[n][al];
+                const double gr = tb.re[n][al], gi = tb.im[n][al];
+                const double2 c = Ck[kk][al * 4 + be];
+                re += gr * c.x - gi * c.y;
+                im += gr * c.y + gi * c.x;
+            }
+            double* o = out + ((((size_t)rhs * 16 + n) * g.T + t) * K + k) * 2;
+            o[0] = re;
+            o[1] = im;
+        }
+        __syncthreads();
+    }
+}
+
+static size_t mom_w2_bytes(const Geo& g, int P, int nrhs)
+{
+    const size_t NP = 2 * P + 1;
+    return round256((size_t)nrhs * g.T * g.Z * NP * NP * 16 * sizeof(double2));
+}
+static size_t mom_smem_bytes(const Geo& g, int P)
+{
+    const size_t NP = 2 * P + 1;
+    return (NP * (g.X + g.Y) + (size_t)MOM_ROWS * g.X * 16 + (size_t)MOM_ROWS * NP * 16) * sizeof(double2);
+}
+
+} // namespace tmk
+
+namespace tmk {
+
+// ---- time dilution -------------------------------------------------------------------------------------------------
+struct TimeMask {
+    unsigned int bits[16]; // T <= 512
+};
+
+// packed full-lattice spinors are arrays [rhs][parity][chunk][cb] of 16-byte chunks (+ fp32 norms for fp16) and a time
+// slice is the contiguous cb range [t V3h, (t+1) V3h): element-wise copy-or-zero.
+__global__ void time_dilute_kernel(Geo g, const char* in, char* out, size_t parity_bytes, int nchunk, int has_norm, TimeMask m)
+{
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cb >= g.Vh) return;
+    const size_t base = (size_t)blockIdx.y * parity_bytes; // blockIdx.y = rhs * 2 + parity
+    const int t = cb / g.V3h;
+    const bool keep = (m.bits[t >> 5] >> (t & 31)) & 1u;
+    const uint4* src = reinterpret_cast<const uint4*>(in + base);
+    uint4* dst = reinterpret_cast<uint4*>(out + base);
+    for (int k = 0; k < nchunk; ++k) dst[(size_t)k * g.Vh + cb] = keep ? src[(size_t)k * g.Vh + cb] : make_uint4(0, 0, 0, 0);
+    if (has_norm) {
+        const float* sn = reinterpret_cast<const float*>(src + (size_t)nchunk * g.Vh);
+        float* dn = reinterpret_cast<float*>(dst + (size_t)nchunk * g.Vh);
+        dn[cb] = keep ? sn[cb] : 0.f;
+    }
+}
+
+// ---- hopping-parameter expansion --------------------------------------------------------------------------------------
+// out_full = (B H) in_full on both parities: B H = -kappa R^-1 Dslash, R^-1 = (1 - i a g5) / (1 + a^2), a = 2 kappa mu
+static int hpe_BH(const Geo& g, const void* gauge, int prec, int recon, void* out_full, const void* in_full, double kappa, double mu,
+                  int nrhs, cudaStream_t st)
+{
+    const size_t pb = spinor_parity_bytes(g, prec);
+    const double a = 2.0 * kappa * mu, d = 1.0 / (1.0 + a * a);
+    DslashParams p;
+    p.gauge = gauge; p.nrhs = nrhs; p.active = nullptr; p.dagger = 0; p.x = nullptr;
+    p.rhs_stride_out = p.rhs_stride_in = p.rhs_stride_x = 2 * pb;
+    p.pq[0] = 0.0; p.pq[1] = 0.0; p.pq[2] = -kappa * d; p.pq[3] = kappa * a * d;
+    for (int parity = 0; parity < 2; ++parity) {
+        p.out = static_cast<char*>(out_full) + parity * pb;
+        p.in = static_cast<const char*>(in_full) + (1 - parity) * pb;
+        p.out_parity = parity;
+        const int rc = launch_dslash(g, prec, recon, p, st);
+        if (rc != TM_OK) return rc;
+    }
+    return TM_OK;
+}
+
+struct C44 {
+    double re[4][4], im[4][4];
+};
+static C44 c44_mul(const C44& a, const C44& b)
+{
+    C44 c = {};
+    for (int i = 0; i < 4; ++i)
+        for (int j = 0; j < 4; ++j)
+            for (int k = 0; k < 4; ++k) {
+                c.re[i][j] += a.re[i][k] * b.re[k][j] - a.im[i][k] * b.im[k][j];
+                c.im[i][j] += a.re[i][k] * b.im[k][j] + a.im[i][k] * b.re[k][j];
+            }
+    return c;
+}
+
+} // namespace tmk
+
+using namespace tmk;
+
+extern "C" int tm_covdev(const tm_lattice* L, const void* gauge, int prec, int recon, void* out_full, const void* in_full, int mu,
+                         int nrhs, void* stream)
+{
+    if (!L || !gauge || !out_full || !in_full || !valid_prec(prec) || !valid_recon(recon)) return TM_ERR_ARG;
+    if (out_full == in_full || mu < 0 || mu > 3 || nrhs < 1) return TM_ERR_ARG;
+    if (!aligned256(gauge) || !aligned256(out_full) || !aligned256(in_full)) return TM_ERR_LAYOUT;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geo& g = L->g;
+    if (prec == 8) return recon == 18 ? covdev_launch<8, 18>(g, gauge, out_full, in_full, mu, nrhs, st) : covdev_launch<8, 12>(g, gauge, out_full, in_full, mu, nrhs, st);
+    if (prec == 4) return recon == 18 ? covdev_launch<4, 18>(g, gauge, out_full, in_full, mu, nrhs, st) : covdev_launch<4, 12>(g, gauge, out_full, in_full, mu, nrhs, st);
+    return recon == 18 ? covdev_launch<2, 18>(g, gauge, out_full, in_full, mu, nrhs, st) : covdev_launch<2, 12>(g, gauge, out_full, in_full, mu, nrhs, st);
+}
+
+extern "C" int tm_contract_field(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, double* out,
+                                 void* stream)
+{
+    if (!L || !a_full || !b_full || !out || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
+    if (!aligned256(a_full) || !aligned256(b_full) || !aligned256(out)) return TM_ERR_LAYOUT;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geo& g = L->g;
+    const size_t pb = spinor_parity_bytes(g, prec);
+    dim3 grid((g.Vh + 127) / 128, 2, nrhs);
+    if (prec == 8) contract_field_kernel<8><<<grid, 128, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, out, L->V);
+    else if (prec == 4) contract_field_kernel<4><<<grid, 128, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, out, L->V);
+    else contract_field_kernel<2><<<grid, 128, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, out, L->V);
+    TM_LAUNCH_CHECK("contract_field_kernel");
+    return TM_OK;
+}
+
+extern "C" size_t tm_loop_momentum_workspace_bytes(const tm_lattice* L, int nrhs, int n_momenta, int pmax)
+{
+    if (!L || nrhs < 1 || n_momenta < 1 || pmax < 0 || pmax > MOM_MAXP) return 0;
+    return round256((size_t)n_momenta * 3 * sizeof(int)) + mom_w2_bytes(L->g, pmax, nrhs);
+}
+
+extern "C" int tm_loop_momentum(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, const int* momenta,
+                                int n_momenta, double* out, void* workspace, size_t workspace_bytes, void* stream)
+{
+    if (!L || !a_full || !b_full || !out || !workspace || !momenta || !valid_prec(prec) || nrhs < 1 || n_momenta < 1) return TM_ERR_ARG;
+    if (!aligned256(a_full) || !aligned256(b_full) || !aligned256(out) || !aligned256(workspace)) return TM_ERR_LAYOUT;
+    int P = 0;
+    for (int i = 0; i < 3 * n_momenta; ++i) P = momenta[i] > P ? momenta[i] : (-momenta[i] > P ? -momenta[i] : P);
+    if (P > MOM_MAXP) return TM_ERR_ARG;
+    if (workspace_bytes < tm_loop_momentum_workspace_bytes(L, nrhs, n_momenta, P)) return TM_ERR_LAYOUT;
+    const Geo& g = L->g;
+    const size_t smem = mom_smem_bytes(g, P);
+    if (smem > 200 * 1024) return TM_ERR_LAYOUT;
+    cudaStream_t st = (cudaStream_t)stream;
+    int* mom_dev = static_cast<int*>(workspace);
+    double2* W2 = reinterpret_cast<double2*>(static_cast<char*>(workspace) + round256((size_t)n_momenta * 3 * sizeof(int)));
+    TM_CUDA_CHECK(cudaMemcpyAsync(mom_dev, momenta, (size_t)n_momenta * 3 * sizeof(int), cudaMemcpyHostToDevice, st));
+    const size_t pb = spinor_parity_bytes(g, prec);
+    dim3 grid(g.Z, g.T, nrhs);
+    if (prec == 8) {
+        TM_CUDA_CHECK(cudaFuncSetAttribute(loop_mom_plane_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        loop_mom_plane_kernel<8><<<grid, MOM_THREADS, smem, st>>>(g, (const char*)a_full, (const char*)b_full, pb, P, W2);
+    } else if (prec == 4) {
+        TM_CUDA_CHECK(cudaFuncSetAttribute(loop_mom_plane_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        loop_mom_plane_kernel<4><<<grid, MOM_THREADS, smem, st>>>(g, (const char*)a_full, (const char*)b_full, pb, P, W2);
+    } else {
+        TM_CUDA_CHECK(cudaFuncSetAttribute(loop_mom_plane_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        loop_mom_plane_kernel<2><<<grid, MOM_THREADS, smem, st>>>(g, (const char*)a_full, (const char*)b_full, pb, P, W2);
+    }
+    TM_LAUNCH_CHECK("loop_mom_plane_kernel");
+    static const GammaTable tb = make_gamma_table();
+    loop_mom_final_kernel<<<dim3(g.T, nrhs), 128, 0, st>>>(g, P, W2, mom_dev, n_momenta, tb, out);
+    TM_LAUNCH_CHECK("loop_mom_final_kernel");
+    return TM_OK;
+}
+
+extern "C" int tm_time_dilute(const tm_lattice* L, const void* in_full, int prec, int nrhs, const unsigned char* keep_slice,
+                              void* out_full, void* stream)
+{
+    if (!L || !in_full || !out_full || !keep_slice || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
+    if (L->g.T > 512) return TM_ERR_LAYOUT;
+    if (!aligned256(in_full) || !aligned256(out_full)) return TM_ERR_LAYOUT;
+    TimeMask m = {};
+    for (int t = 0; t < L->g.T; ++t)
+        if (keep_slice[t]) m.bits[t >> 5] |= 1u << (t & 31);
+    const Geo& g = L->g;
+    const int nchunk = 24 * prec / 16;
+    dim3 grid((g.Vh + 255) / 256, 2 * nrhs);
+    time_dilute_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(g, (const char*)in_full, (char*)out_full, spinor_parity_bytes(g, prec),
+                                                               nchunk, prec == 2, m);
+    TM_LAUNCH_CHECK("time_dilute_kernel");
+    return TM_OK;
+}
+
+extern "C" int tm_hpe_remainder(const tm_lattice* L, const void* gauge, int prec, int recon, void* out_full, const void* s_full,
+                                void* tmp_full, double kappa, double mu, int nrhs, void* stream)
+{
+    if (!L || !gauge || !out_full || !s_full || !tmp_full || !valid_prec(prec) || !valid_recon(recon)) return TM_ERR_ARG;
+    if (out_full == s_full || tmp_full == s_full || tmp_full == out_full || nrhs < 1 || nrhs > TM_MAX_NRHS) return TM_ERR_ARG;
+    if (!aligned256(gauge) || !aligned256(out_full) || !aligned256(s_full) || !aligned256(tmp_full)) return TM_ERR_LAYOUT;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geo& g = L->g;
+    int rc = hpe_BH(g, gauge, prec, recon, tmp_full, s_full, kappa, mu, nrhs, st);
+    if (rc == TM_OK) rc = hpe_BH(g, gauge, prec, recon, out_full, tmp_full, kappa, mu, nrhs, st);
+    if (rc == TM_OK) rc = hpe_BH(g, gauge, prec, recon, tmp_full, out_full, kappa, mu, nrhs, st);
+    if (rc == TM_OK) rc = hpe_BH(g, gauge, prec, recon, out_full, tmp_full, kappa, mu, nrhs, st);
+    return rc;
+}
+
+extern "C" int tm_hpe_local_traces(double kappa, double mu, double* out16)
+{
+    if (!out16) return TM_ERR_ARG;
+    // host arithmetic on 4x4 complex matrices: S = B + kappa^2 sum_mu [B (1-g) B (1+g) B + B (1+g) B (1-g) B], B = R^-1
+    const double a = 2.0 * kappa * mu, d = 1.0 / (1.0 + a * a);
+    GammaZ gm[4][4][4];
+    gamma_mu_table(gm);
+    C44 B = {};
+    for (int i = 0; i < 4; ++i) {
+        B.re[i][i] = d;
+        B.im[i][i] = (i < 2 ? -a : a) * d; // (1 - i a g5)/(1 + a^2), g5 = diag(1,1,-1,-1)
+    }
+    C44 S = B;
+    for (int m = 0; m < 4; ++m)
+        for (int sg = -1; sg <= 1; sg += 2) {
+            C44 Pm = {}, Pp = {};
+            for (int i = 0; i < 4; ++i)
+                for (int j = 0; j < 4; ++j) {
+                    Pm.re[i][j] = (i == j) - sg * gm[m][i][j].re;
+                    Pm.im[i][j] = -sg * gm[m][i][j].im;
+                    Pp.re[i][j] = (i == j) + sg * gm[m][i][j].re;
+                    Pp.im[i][j] = sg * gm[m][i][j].im;
+                }
+            const C44 t = c44_mul(c44_mul(c44_mul(c44_mul(B, Pm), B), Pp), B);
+            for (int i = 0; i < 4; ++i)
+                for (int j = 0; j < 4; ++j) {
+                    S.re[i][j] += kappa * kappa * t.re[i][j];
+                    S.im[i][j] += kappa * kappa * t.im[i][j];
+                }
+        }
+    const GammaTable tb = make_gamma_table();
+    for (int n = 0; n < 16; ++n) {
+        double re = 0.0, im = 0.0; // 3 tr[Gamma_n S] = 3 sum_al Gamma_n[al][col] S[col][al]
+        for (int al = 0; al < 4; ++al) {
+            const int be = tb.col[n][al];
+            re += tb.re[n][al] * S.re[be][al] - tb.im[n][al] * S.im[be][al];
+            im += tb.re[n][al] * S.im[be][al] + tb.im[n][al] * S.re[be][al];
+        }
+        out16[2 * n] = 3.0 * re;
+        out16[2 * n + 1] = 3.0 * im;
+    }
+    return TM_OK;
+}

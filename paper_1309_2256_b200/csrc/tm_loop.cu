@@ -10,66 +10,20 @@
 // at most LOOP_CHUNK = 8 sites of a thread, then fp64: per-thread accumulator, warp shuffles, shared memory across warps, per-block partials, then one fixed-order final pass:
 // bit-reproducible, no floating-point atomics.
 #include "tm_layout.cuh"
+#include "tm_gamma.cuh"
 
 namespace tmk {
-
-struct GammaTable {
-    // Gamma_n has one non-zero entry per row: (Gamma_n)_{al, col[n][al]} = re + i im, entries in {+-1, +-i}
-    signed char col[16][4], re[16][4], im[16][4];
-};
-
-// own gamma table (chiral basis of include/tm.h), multiplied out in integer arithmetic on the host
-static GammaTable make_gamma_table()
-{
-    struct Z { int re, im; };
-    auto mul = [](Z a, Z b) { return Z{a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; };
-    Z g[4][4][4] = {};
-    // g_k = [[0, -i s_k], [i s_k, 0]], g_4 = [[0, 1], [1, 0]]
-    const Z s[3][2][2] = {{{{0, 0}, {1, 0}}, {{1, 0}, {0, 0}}}, {{{0, 0}, {0, -1}}, {{0, 1}, {0, 0}}}, {{{1, 0}, {0, 0}}, {{0, 0}, {-1, 0}}}};
-    for (int k = 0; k < 3; ++k)
-        for (int a = 0; a < 2; ++a)
-            for (int b = 0; b < 2; ++b) {
-                g[k][a][2 + b] = mul(Z{0, -1}, s[k][a][b]);
-                g[k][2 + a][b] = mul(Z{0, 1}, s[k][a][b]);
-            }
-    g[3][0][2] = g[3][1][3] = g[3][2][0] = g[3][3][1] = Z{1, 0};
-    GammaTable tb;
-    for (int n = 0; n < 16; ++n) {
-        Z p[4][4] = {};
-        for (int a = 0; a < 4; ++a) p[a][a] = Z{1, 0};
-        for (int k = 0; k < 4; ++k) {
-            if (!((n >> k) & 1)) continue;
-            Z q[4][4] = {};
-            for (int a = 0; a < 4; ++a)
-                for (int b = 0; b < 4; ++b)
-                    for (int c = 0; c < 4; ++c) {
-                        const Z m = mul(p[a][c], g[k][c][b]);
-                        q[a][b].re += m.re;
-                        q[a][b].im += m.im;
-                    }
-            for (int a = 0; a < 4; ++a)
-                for (int b = 0; b < 4; ++b) p[a][b] = q[a][b];
-        }
-        for (int a = 0; a < 4; ++a)
-            for (int b = 0; b < 4; ++b)
-                if (p[a][b].re != 0 || p[a][b].im != 0) {
-                    tb.col[n][a] = (signed char)b;
-                    tb.re[n][a] = (signed char)p[a][b].re;
-                    tb.im[n][a] = (signed char)p[a][b].im;
-                }
-    }
-    return tb;
-}
 
 constexpr int LOOP_THREADS = 128;
 constexpr int LOOP_CHUNK = 8; // sites summed in the storage arithmetic before the fp64 accumulator takes over
 
 template <int PREC>
 __global__ void __launch_bounds__(LOOP_THREADS) loop_partial_kernel(Geo g, const char* a_full, const char* b_full,
-                                                                    size_t parity_bytes, double* partial, int nb)
+                                                                    size_t parity_bytes, double* partial, int nb, int t0)
 {
     typedef typename Prec<PREC>::real real;
-    const int t = blockIdx.y, rhs = blockIdx.z;
+    const int t = t0 + blockIdx.y, rhs = blockIdx.z; // gridDim.y time slices starting at t0
+
     const char* af = a_full + (size_t)rhs * 2 * parity_bytes;
     const char* bf = b_full + (size_t)rhs * 2 * parity_bytes;
     // per-thread partial sums: products and the sum over up to LOOP_CHUNK sites in the storage arithmetic, then fp64
@@ -130,7 +84,7 @@ __global__ void __launch_bounds__(LOOP_THREADS) loop_partial_kernel(Geo g, const
         double v = 0.0;
 #pragma unroll
         for (int w = 0; w < LOOP_THREADS / 32; ++w) v += sm[w][threadIdx.x];
-        partial[(((size_t)rhs * g.T + t) * nb + blockIdx.x) * 32 + threadIdx.x] = v;
+        partial[(((size_t)rhs * gridDim.y + blockIdx.y) * nb + blockIdx.x) * 32 + threadIdx.x] = v;
     }
 }
 
@@ -173,21 +127,28 @@ static int loop_nb(const Geo& g)
     return nb;
 }
 
-int loop_contract_ex(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,
-                     int g5_left, int g5_right, double scale_re, double scale_im, cudaStream_t st)
+// time slices [t0, t0 + nt): out[rhs][16][nt][2]
+int loop_contract_range(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,
+                        int g5_left, int g5_right, double scale_re, double scale_im, int t0, int nt, cudaStream_t st)
 {
     static const GammaTable tb = make_gamma_table();
     const int nb = loop_nb(g);
-    dim3 grid(nb, g.T, nrhs), block(LOOP_THREADS);
+    dim3 grid(nb, nt, nrhs), block(LOOP_THREADS);
     const size_t pb = spinor_parity_bytes(g, prec);
     double* partial = static_cast<double*>(workspace);
-    if (prec == 8) loop_partial_kernel<8><<<grid, block, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, partial, nb);
-    else if (prec == 4) loop_partial_kernel<4><<<grid, block, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, partial, nb);
-    else loop_partial_kernel<2><<<grid, block, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, partial, nb);
+    if (prec == 8) loop_partial_kernel<8><<<grid, block, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, partial, nb, t0);
+    else if (prec == 4) loop_partial_kernel<4><<<grid, block, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, partial, nb, t0);
+    else loop_partial_kernel<2><<<grid, block, 0, st>>>(g, (const char*)a_full, (const char*)b_full, pb, partial, nb, t0);
     TM_LAUNCH_CHECK("loop_partial_kernel");
-    loop_final_kernel<<<dim3(g.T, nrhs), 32, 0, st>>>(g.T, nb, partial, tb, out, g5_left, g5_right, scale_re, scale_im);
+    loop_final_kernel<<<dim3(nt, nrhs), 32, 0, st>>>(nt, nb, partial, tb, out, g5_left, g5_right, scale_re, scale_im);
     TM_LAUNCH_CHECK("loop_final_kernel");
     return TM_OK;
+}
+
+int loop_contract_ex(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,
+                     int g5_left, int g5_right, double scale_re, double scale_im, cudaStream_t st)
+{
+    return loop_contract_range(g, a_full, b_full, prec, nrhs, out, workspace, g5_left, g5_right, scale_re, scale_im, 0, g.T, st);
 }
 
 int loop_contract(const Geo& g, const void* a_full, const void* b_full, int prec, int nrhs, double* out, void* workspace,
@@ -223,4 +184,14 @@ extern "C" int tm_loop_contract_ex(const tm_lattice* L, const void* a_full, cons
     if (!aligned256(a_full) || !aligned256(b_full) || !aligned256(out) || !aligned256(workspace)) return TM_ERR_LAYOUT;
     return loop_contract_ex(L->g, a_full, b_full, prec, nrhs, out, workspace, g5_left != 0, g5_right != 0, scale_re, scale_im,
                             (cudaStream_t)stream);
+}
+
+/* single-time-slice contraction, used with time-diluted sources */
+extern "C" int tm_loop_contract_slice(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, int t0,
+                                      double* out, void* workspace, void* stream)
+{
+    if (!L || !a_full || !b_full || !out || !workspace || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
+    if (t0 < 0 || t0 >= L->g.T) return TM_ERR_ARG;
+    if (!aligned256(a_full) || !aligned256(b_full) || !aligned256(out) || !aligned256(workspace)) return TM_ERR_LAYOUT;
+    return loop_contract_range(L->g, a_full, b_full, prec, nrhs, out, workspace, 0, 0, 1.0, 0.0, t0, 1, (cudaStream_t)stream);
 }
