@@ -331,6 +331,46 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
     f(0)
     ms = time_events(torch, f, 10)
     out["loop_contract_fp16_x12"] = {"us": ms * 1e3, "GBps_algorithmic": 2 * fb / ms / 1e6, "frac_of_measured": 2 * fb / ms / 1e6 / hbm_peak}
+    # NEXT-2 / NEXT-3 rows at 32^3x64: momentum-projected loops for the p^2 <= 9 list (123 momenta), the
+    # contraction field, the covariant derivative and the HPE remainder; algorithmic bytes as for the loop kernel
+    ins = {}
+    r = int(np.floor(np.sqrt(9)))
+    mom = np.array([(x, y, z) for x in range(-r, r + 1) for y in range(-r, r + 1) for z in range(-r, r + 1) if x * x + y * y + z * z <= 9],
+                   dtype=np.int32)
+    lm = torch.zeros((NRHS, 16, DIMS[3], len(mom), 2), dtype=torch.float64, device="cuda")
+    mws = tm.device_buffer(tm.tm_loop_momentum_workspace_bytes(L, NRHS, len(mom), r))
+    f = lambda i: tm.tm_loop_momentum(L, a, b, prec, NRHS, mom, lm, mws)
+    f(0)
+    ms = time_events(torch, f, 5)
+    ins["loop_momentum_p2le9_fp16_x12"] = {"us": ms * 1e3, "momenta": int(len(mom)), "GBps_algorithmic": 2 * fb / ms / 1e6,
+                                           "frac_of_measured": 2 * fb / ms / 1e6 / hbm_peak}
+    del lm, mws
+    fb1 = tm.tm_spinor_bytes(L, prec, 1, 1)
+    cf = torch.empty((L.V, 32), dtype=torch.float64, device="cuda")
+    f = lambda i: tm.tm_contract_field(L, a, b, prec, 1, cf)
+    f(0)
+    ms = time_events(torch, f, 10)
+    by = 2 * fb1 + L.V * 256
+    ins["contract_field_fp16"] = {"us": ms * 1e3, "GBps_algorithmic": by / ms / 1e6, "frac_of_measured": by / ms / 1e6 / hbm_peak}
+    del cf
+    for p_, rc_ in ((4, 18), (2, 12)):
+        fbp = tm.tm_spinor_bytes(L, p_, 1, 1)
+        vin, vout, vtmp = tm.device_buffer(fbp), tm.device_buffer(fbp), tm.device_buffer(fbp)
+        tm.tm_spinor_pack(L, psi, p_, 1, vin)
+        f = lambda i: tm.tm_covdev(L, gauges[(p_, rc_)], p_, rc_, vout, vin, i % 4, 1)
+        f(0)
+        ms = time_events(torch, f, 20)
+        by = L.V * rc_ * p_ + 2 * fbp  # one link per site (each link serves a forward and a backward hop), spinor in + out
+        ins["covdev_fp%d_recon%d" % (8 * p_, rc_)] = {"us": ms * 1e3, "GBps_algorithmic": by / ms / 1e6,
+                                                     "frac_of_measured": by / ms / 1e6 / hbm_peak}
+        f = lambda i: tm.tm_hpe_remainder(L, gauges[(p_, rc_)], p_, rc_, vout, vin, vtmp, kappa, mu, 1)
+        f(0)
+        ms = time_events(torch, f, 5)
+        by = 8 * dslash_bytes(Vh, p_, rc_, False)
+        ins["hpe_remainder_fp%d_recon%d" % (8 * p_, rc_)] = {"us": ms * 1e3, "launches": 8, "GBps_algorithmic": by / ms / 1e6,
+                                                            "frac_of_measured": by / ms / 1e6 / hbm_peak}
+        del vin, vout, vtmp
+    out["insertions_next2_next3"] = ins
     del a, b
 
     # mixed-precision CG to 1e-8 on one Z2xiZ2 source (configs[2]): fp64 reliable updates, fp32 and fp16 iterations

@@ -125,11 +125,9 @@ namespace tmk {
 //     W2[rhs][t][z][ipx][ipy][ab] = sum_y e^{-2 pi i n_y y / Y} sum_x e^{-2 pi i n_x x / X} C_ab(x, y, z, t).
 // Stage 2 (loop_mom_final_kernel): DFT over z for the listed momenta and the 16 Gamma_n.
 constexpr int MOM_THREADS = 256;
-constexpr int MOM_ROWS = 4;   // y rows contracted per pass
+constexpr int MOM_ROWS = 8;   // y rows contracted per pass (at most; MOM_THREADS / X when X > 32)
 constexpr int MOM_MAXP = 4;   // |n_i| <= 4 (p^2 <= 9 needs 3)
-constexpr int MOM_ACC = (2 * MOM_MAXP + 1) * (2 * MOM_MAXP + 1) * 16 / MOM_THREADS + 1;
 
-__device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 __device__ __forceinline__ double2 cfma(double2 a, double2 b, double2 c)
 {
     return make_double2(fma(a.x, b.x, fma(-a.y, b.y, c.x)), fma(a.x, b.y, fma(a.y, b.x, c.y)));
@@ -143,31 +141,57 @@ __device__ __forceinline__ double2 dft_phase(int n, int k, int N)
     sincospi(-2.0 * (double)m / (double)N, &s, &c);
     return make_double2(c, s);
 }
+// (cos, sin)(2 pi n k / N)
+__device__ __forceinline__ double2 cos_sin(int n, int k, int N)
+{
+    double s, c;
+    sincospi(2.0 * (double)((n * k) % N) / (double)N, &s, &c);
+    return make_double2(c, s);
+}
 
-template <int PREC>
-__global__ void __launch_bounds__(MOM_THREADS) loop_mom_plane_kernel(Geo g, const char* a_full, const char* b_full,
-                                                                     size_t parity_bytes, int P, double2* W2)
+template <int PREC> struct MomC { typedef float2 type; };
+template <> struct MomC<8> { typedef double2 type; };
+
+// e^{-i n theta} = cos(n theta) - i sin(n theta): the sums over x (and y) are kept as real-weighted sums
+//   Sc[n] = sum C cos(n theta), Ss[n] = sum C sin(n theta), n = 0..P, and +-n are combined at the end (half the multiplies
+// of a complex DFT).  Every thread keeps its 2 P + 1 complex sums in registers and reads each C once.
+template <int PREC, int P>
+__global__ void __launch_bounds__(MOM_THREADS, PREC == 8 ? 2 : 3) loop_mom_plane_kernel(Geo g, const char* a_full, const char* b_full,
+                                                                     size_t parity_bytes, int R, double2* W2)
 {
     typedef typename Prec<PREC>::real real;
+    typedef typename MomC<PREC>::type CT;
     extern __shared__ double2 smem[];
-    const int X = g.X, Y = g.Y, NP = 2 * P + 1;
-    double2* ex = smem;                      // [NP][X]
-    double2* ey = ex + NP * X;               // [NP][Y]
-    double2* Cs = ey + NP * Y;               // [MOM_ROWS][X][16]
-    double2* W1 = Cs + MOM_ROWS * X * 16;    // [MOM_ROWS][NP][16]
+    constexpr int NP = 2 * P + 1;
+    const int X = g.X, Y = g.Y;
+    // x sums run in the storage arithmetic (fp32 for fp32 / fp16 fields: at most X terms per sum, like the LOOP_CHUNK sites of
+    // loop_partial_kernel), everything after them in fp64
+    typedef typename Prec<PREC>::real acc_t;
+    double2* csy = smem;                          // [P+1][Y]  (cos, sin)(2 pi n y / Y)
+    double2* Part = csy + (P + 1) * Y;            // [nseg][R][16][NP]
+    const int nseg = max(1, MOM_THREADS / (R * 16));
+    const int nh = min(4, MOM_THREADS / (NP * 16)); // row shares of step (3); Part also serves as their [nh][NP*16][NP] scratch
+    CT* csx = reinterpret_cast<CT*>(Part + (size_t)max(nseg * R, nh * NP) * 16 * NP); // [P+1][X]
+    CT* Cs = csx + (P + 1) * X;                   // [R][X][16]
     const int z = blockIdx.x, t = blockIdx.y, rhs = blockIdx.z, tid = threadIdx.x;
-    for (int i = tid; i < NP * X; i += MOM_THREADS) ex[i] = dft_phase(i / X - P, i % X, X);
-    for (int i = tid; i < NP * Y; i += MOM_THREADS) ey[i] = dft_phase(i / Y - P, i % Y, Y);
-    double2 acc[MOM_ACC];
+    for (int i = tid; i < (P + 1) * X; i += MOM_THREADS) {
+        const double2 w = cos_sin(i / X, i % X, X);
+        CT v;
+        v.x = (acc_t)w.x;
+        v.y = (acc_t)w.y;
+        csx[i] = v;
+    }
+    for (int i = tid; i < (P + 1) * Y; i += MOM_THREADS) csy[i] = cos_sin(i / Y, i % Y, Y);
+    double2 yc[P + 1], ys[P + 1];
 #pragma unroll
-    for (int j = 0; j < MOM_ACC; ++j) acc[j] = make_double2(0.0, 0.0);
-    const int nout = NP * NP * 16;
+    for (int m = 0; m <= P; ++m) yc[m] = ys[m] = make_double2(0.0, 0.0);
     const char* af = a_full + (size_t)rhs * 2 * parity_bytes;
     const char* bf = b_full + (size_t)rhs * 2 * parity_bytes;
+    const int xseg = (X + nseg - 1) / nseg;
     __syncthreads();
-    for (int y0 = 0; y0 < Y; y0 += MOM_ROWS) {
-        const int nr = min(MOM_ROWS, Y - y0);
-        // (1) contraction of the sites of rows y0 .. y0 + nr - 1
+    for (int y0 = 0; y0 < Y; y0 += R) {
+        const int nr = min(R, Y - y0);
+        // (1) contraction of the sites of rows y0 .. y0 + nr - 1, products in the storage arithmetic
         for (int i = tid; i < nr * X; i += MOM_THREADS) {
             const int r = i / X, x = i - r * X, y = y0 + r;
             const int parity = (x + y + z + t) & 1;
@@ -177,37 +201,114 @@ __global__ void __launch_bounds__(MOM_THREADS) loop_mom_plane_kernel(Geo g, cons
             load_spinor<PREC>(bf + (size_t)parity * parity_bytes, g.Vh, cb, b);
             site_contract<real>(a, b, c);
 #pragma unroll
-            for (int k = 0; k < 16; ++k) Cs[(r * X + x) * 16 + k] = make_double2((double)c[2 * k], (double)c[2 * k + 1]);
-        }
-        __syncthreads();
-        // (2) DFT over x
-        for (int o = tid; o < nr * NP * 16; o += MOM_THREADS) {
-            const int ab = o & 15, ip = (o >> 4) % NP, r = (o >> 4) / NP;
-            double2 s = make_double2(0.0, 0.0);
-            for (int x = 0; x < X; ++x) s = cfma(Cs[(r * X + x) * 16 + ab], ex[ip * X + x], s);
-            W1[(r * NP + ip) * 16 + ab] = s;
-        }
-        __syncthreads();
-        // (3) DFT over y, accumulated
-#pragma unroll
-        for (int j = 0; j < MOM_ACC; ++j) {
-            const int o = tid + j * MOM_THREADS;
-            if (o < nout) {
-                const int ab = o & 15, ipy = (o >> 4) % NP, ipx = (o >> 4) / NP;
-                for (int r = 0; r < nr; ++r) acc[j] = cfma(W1[(r * NP + ipx) * 16 + ab], ey[ipy * Y + y0 + r], acc[j]);
+            for (int k = 0; k < 16; ++k) {
+                CT v;
+                v.x = c[2 * k];
+                v.y = c[2 * k + 1];
+                Cs[(r * X + x) * 16 + k] = v;
             }
         }
         __syncthreads();
-    }
-    double2* dst = W2 + (((size_t)rhs * g.T + t) * g.Z + z) * nout;
+        // (2) sums over x: thread = (segment of x, row, ab)
+        if (tid < nseg * R * 16) {
+            const int ab = tid & 15, r = (tid >> 4) % R, seg = (tid >> 4) / R;
+            if (r < nr) {
+                acc_t scx[P + 1], scy[P + 1], ssx[P + 1], ssy[P + 1];
 #pragma unroll
-    for (int j = 0; j < MOM_ACC; ++j) {
-        const int o = tid + j * MOM_THREADS;
-        if (o < nout) dst[o] = acc[j];
+                for (int n = 0; n <= P; ++n) scx[n] = scy[n] = ssx[n] = ssy[n] = 0;
+                const int x1 = min(X, (seg + 1) * xseg);
+#pragma unroll 4
+                for (int x = seg * xseg; x < x1; ++x) {
+                    const CT cv = Cs[(r * X + x) * 16 + ab];
+#pragma unroll
+                    for (int n = 0; n <= P; ++n) {
+                        const CT w = csx[n * X + x];
+                        scx[n] = fma(cv.x, w.x, scx[n]);
+                        scy[n] = fma(cv.y, w.x, scy[n]);
+                        if (n > 0) {
+                            ssx[n] = fma(cv.x, w.y, ssx[n]);
+                            ssy[n] = fma(cv.y, w.y, ssy[n]);
+                        }
+                    }
+                }
+                double2* dst = Part + (size_t)((seg * R + r) * 16 + ab) * NP;
+#pragma unroll
+                for (int n = 0; n <= P; ++n)
+                    if (n <= P) {
+                        dst[n] = make_double2((double)scx[n], (double)scy[n]);
+                        if (n > 0) dst[P + n] = make_double2((double)ssx[n], (double)ssy[n]);
+                    }
+            }
+        }
+        __syncthreads();
+        // (3) sums over y: thread = (share of the rows, ipx, ab); W1 = sum_seg [Sc[|n|] - sgn(n) i Ss[|n|]].  No barrier after
+        // this step: the next pass's contraction only writes Cs, and Part is rewritten after the next barrier.
+        if (tid < nh * NP * 16) {
+            const int item = tid % (NP * 16), half = tid / (NP * 16);
+            const int ab = item & 15, n = (item >> 4) - P, an = n < 0 ? -n : n;
+            const double sg = n > 0 ? 1.0 : (n < 0 ? -1.0 : 0.0);
+            for (int r = half; r < nr; r += nh) {
+                double2 w = make_double2(0.0, 0.0);
+                for (int seg = 0; seg < nseg; ++seg) {
+                    const double2* src = Part + (size_t)((seg * R + r) * 16 + ab) * NP;
+                    const double2 c = src[an];
+                    w.x += c.x;
+                    w.y += c.y;
+                    if (an > 0) {
+                        const double2 sn = src[P + an];
+                        w.x += sg * sn.y; // -i sg (sx + i sy) = sg sy - i sg sx
+                        w.y -= sg * sn.x;
+                    }
+                }
+#pragma unroll
+                for (int m = 0; m <= P; ++m) {
+                    const double2 q = csy[m * Y + y0 + r];
+                    yc[m].x = fma(w.x, q.x, yc[m].x);
+                    yc[m].y = fma(w.y, q.x, yc[m].y);
+                    if (m > 0) {
+                        ys[m].x = fma(w.x, q.y, ys[m].x);
+                        ys[m].y = fma(w.y, q.y, ys[m].y);
+                    }
+                }
+            }
+        }
+    }
+    // combine the row shares in a fixed order (Part is free again after this barrier)
+    __syncthreads();
+    if (tid < nh * NP * 16) {
+        double2* dst = Part + (size_t)tid * NP;
+#pragma unroll
+        for (int m = 0; m <= P; ++m) {
+            dst[m] = yc[m];
+            if (m > 0) dst[P + m] = ys[m];
+        }
+    }
+    __syncthreads();
+    if (tid < NP * 16) {
+        for (int h = 1; h < nh; ++h) {
+            const double2* src = Part + (size_t)(h * NP * 16 + tid) * NP;
+#pragma unroll
+            for (int m = 0; m <= P; ++m) {
+                yc[m].x += src[m].x;
+                yc[m].y += src[m].y;
+                if (m > 0) {
+                    ys[m].x += src[P + m].x;
+                    ys[m].y += src[P + m].y;
+                }
+            }
+        }
+        const int ab = tid & 15, ipx = tid >> 4;
+        double2* dst = W2 + (((size_t)rhs * g.T + t) * g.Z + z) * (NP * NP * 16);
+#pragma unroll
+        for (int m = 0; m <= P; ++m) {
+            // n_y = +m: Yc - i Ys ; n_y = -m: Yc + i Ys
+            dst[(ipx * NP + (P + m)) * 16 + ab] = make_double2(yc[m].x + ys[m].y, yc[m].y - ys[m].x);
+            if (m > 0) dst[(ipx * NP + (P - m)) * 16 + ab] = make_double2(yc[m].x - ys[m].y, yc[m].y + ys[m].x);
+        }
     }
 }
 
-// out[rhs][n][t][k] = sum_ab (Gamma_n)_ab sum_z e^{-2 pi i n_z z / Z} W2[rhs][t][z][ipx_k][ipy_k][ab]
+// out[rhs][n][t][k] = sum_ab (Gamma_n)_ab sum_z e^{-2 pi i n_z z / Z} W2[rhs][t][z][ipx_k][ipy_k][ab]; 8 momenta per CTA
 __global__ void __launch_bounds__(128) loop_mom_final_kernel(Geo g, int P, const double2* W2, const int* mom, int K, GammaTable tb,
                                                              double* out)
 {
@@ -215,32 +316,29 @@ __global__ void __launch_bounds__(128) loop_mom_final_kernel(Geo g, int P, const
     const int t = blockIdx.x, rhs = blockIdx.y;
     const int NP = 2 * P + 1, nout = NP * NP * 16;
     const int kk = threadIdx.x >> 4, ab = threadIdx.x & 15;
-    for (int k0 = 0; k0 < K; k0 += 8) {
-        const int k = k0 + kk;
-        if (k < K) {
-            const int nx = mom[3 * k], ny = mom[3 * k + 1], nz = mom[3 * k + 2];
-            const double2* src = W2 + ((size_t)rhs * g.T + t) * g.Z * nout + ((nx + P) * NP + (ny + P)) * 16 + ab;
-            double2 s = make_double2(0.0, 0.0);
-            for (int z = 0; z < g.Z; ++z) s = cfma(src[(size_t)z * nout], dft_phase(nz, z, g.Z), s);
-            Ck[kk][ab] = s;
-        }
-        __syncthreads();
-        if (k < K) {
-            const int n = ab;
-            double re = 0.0, im = 0.0;
+    const int k = blockIdx.z * 8 + kk;
+    if (k < K) {
+        const int nx = mom[3 * k], ny = mom[3 * k + 1], nz = mom[3 * k + 2];
+        const double2* src = W2 + ((size_t)rhs * g.T + t) * g.Z * nout + ((nx + P) * NP + (ny + P)) * 16 + ab;
+        double2 s = make_double2(0.0, 0.0);
+        for (int z = 0; z < g.Z; ++z) s = cfma(src[(size_t)z * nout], dft_phase(nz, z, g.Z), s);
+        Ck[kk][ab] = s;
+    }
+    __syncthreads();
+    if (k < K) {
+        const int n = ab;
+        double re = 0.0, im = 0.0;
 #pragma unroll
-            for (int al = 0; al < 4; ++al) {
-                const int be = tb.col[n][al];
-                const double gr = tb.re[n][al], gi = tb.im[n][al];
-                const double2 c = Ck[kk][al * 4 + be];
-                re += gr * c.x - gi * c.y;
-                im += gr * c.y + gi * c.x;
-            }
-            double* o = out + ((((size_t)rhs * 16 + n) * g.T + t) * K + k) * 2;
-            o[0] = re;
-            o[1] = im;
+        for (int al = 0; al < 4; ++al) {
+            const int be = tb.col[n][al];
+            const double gr = tb.re[n][al], gi = tb.im[n][al];
+            const double2 c = Ck[kk][al * 4 + be];
+            re += gr * c.x - gi * c.y;
+            im += gr * c.y + gi * c.x;
         }
-        __syncthreads();
+        double* o = out + ((((size_t)rhs * 16 + n) * g.T + t) * K + k) * 2;
+        o[0] = re;
+        o[1] = im;
     }
 }
 
@@ -249,10 +347,22 @@ static size_t mom_w2_bytes(const Geo& g, int P, int nrhs)
     const size_t NP = 2 * P + 1;
     return round256((size_t)nrhs * g.T * g.Z * NP * NP * 16 * sizeof(double2));
 }
-static size_t mom_smem_bytes(const Geo& g, int P)
+static int mom_rows(const Geo& g)
 {
-    const size_t NP = 2 * P + 1;
-    return (NP * (g.X + g.Y) + (size_t)MOM_ROWS * g.X * 16 + (size_t)MOM_ROWS * NP * 16) * sizeof(double2);
+    int R = MOM_THREADS / g.X;
+    if (R > MOM_ROWS) R = MOM_ROWS;
+    if (R < 1) R = 1;
+    if (R > g.Y) R = g.Y;
+    return R;
+}
+static size_t mom_smem_bytes(const Geo& g, int P, int prec)
+{
+    const size_t NP = 2 * P + 1, R = mom_rows(g);
+    const size_t nseg = MOM_THREADS / (R * 16) > 0 ? MOM_THREADS / (R * 16) : 1;
+    size_t nh = MOM_THREADS / (NP * 16);
+    if (nh > 4) nh = 4;
+    const size_t part = (nseg * R > nh * NP ? nseg * R : nh * NP) * 16 * NP;
+    return ((size_t)(P + 1) * g.Y + part) * sizeof(double2) + ((size_t)(P + 1) * g.X + R * g.X * 16) * (prec == 8 ? sizeof(double2) : sizeof(float2));
 }
 
 } // namespace tmk
@@ -368,7 +478,8 @@ extern "C" int tm_loop_momentum(const tm_lattice* L, const void* a_full, const v
     if (P > MOM_MAXP) return TM_ERR_ARG;
     if (workspace_bytes < tm_loop_momentum_workspace_bytes(L, nrhs, n_momenta, P)) return TM_ERR_LAYOUT;
     const Geo& g = L->g;
-    const size_t smem = mom_smem_bytes(g, P);
+    const size_t smem = mom_smem_bytes(g, P, prec);
+    const int R = mom_rows(g);
     if (smem > 200 * 1024) return TM_ERR_LAYOUT;
     cudaStream_t st = (cudaStream_t)stream;
     int* mom_dev = static_cast<int*>(workspace);
@@ -376,19 +487,29 @@ extern "C" int tm_loop_momentum(const tm_lattice* L, const void* a_full, const v
     TM_CUDA_CHECK(cudaMemcpyAsync(mom_dev, momenta, (size_t)n_momenta * 3 * sizeof(int), cudaMemcpyHostToDevice, st));
     const size_t pb = spinor_parity_bytes(g, prec);
     dim3 grid(g.Z, g.T, nrhs);
+#define TM_MOM_LAUNCH(PR, PP)                                                                                                   \
+    do {                                                                                                                        \
+        TM_CUDA_CHECK(cudaFuncSetAttribute(loop_mom_plane_kernel<PR, PP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        loop_mom_plane_kernel<PR, PP><<<grid, MOM_THREADS, smem, st>>>(g, (const char*)a_full, (const char*)b_full, pb, R, W2);   \
+    } while (0)
+#define TM_MOM_SWITCH(PR)                                                                                                       \
+    switch (P) {                                                                                                                \
+    case 0: TM_MOM_LAUNCH(PR, 0); break;                                                                                        \
+    case 1: TM_MOM_LAUNCH(PR, 1); break;                                                                                        \
+    case 2: TM_MOM_LAUNCH(PR, 2); break;                                                                                        \
+    case 3: TM_MOM_LAUNCH(PR, 3); break;                                                                                        \
+    default: TM_MOM_LAUNCH(PR, 4); break;                                                                                       \
+    }
     if (prec == 8) {
-        TM_CUDA_CHECK(cudaFuncSetAttribute(loop_mom_plane_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        loop_mom_plane_kernel<8><<<grid, MOM_THREADS, smem, st>>>(g, (const char*)a_full, (const char*)b_full, pb, P, W2);
+        TM_MOM_SWITCH(8)
     } else if (prec == 4) {
-        TM_CUDA_CHECK(cudaFuncSetAttribute(loop_mom_plane_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        loop_mom_plane_kernel<4><<<grid, MOM_THREADS, smem, st>>>(g, (const char*)a_full, (const char*)b_full, pb, P, W2);
+        TM_MOM_SWITCH(4)
     } else {
-        TM_CUDA_CHECK(cudaFuncSetAttribute(loop_mom_plane_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        loop_mom_plane_kernel<2><<<grid, MOM_THREADS, smem, st>>>(g, (const char*)a_full, (const char*)b_full, pb, P, W2);
+        TM_MOM_SWITCH(2)
     }
     TM_LAUNCH_CHECK("loop_mom_plane_kernel");
     static const GammaTable tb = make_gamma_table();
-    loop_mom_final_kernel<<<dim3(g.T, nrhs), 128, 0, st>>>(g, P, W2, mom_dev, n_momenta, tb, out);
+    loop_mom_final_kernel<<<dim3(g.T, nrhs, (n_momenta + 7) / 8), 128, 0, st>>>(g, P, W2, mom_dev, n_momenta, tb, out);
     TM_LAUNCH_CHECK("loop_mom_final_kernel");
     return TM_OK;
 }
