@@ -155,7 +155,7 @@ def run_b200(args, rank, world, local_rank):
     # ---- once per configuration: gauge field -> packed links (a0) ----
     U = torch.from_numpy(ti.gauge(DIMS).view(np.float64)).cuda()
     gauges = {}
-    for prec, recon in ((2, 12), (2, 18), (4, 12), (4, 18), (8, 12)):
+    for prec, recon in ((2, 12), (2, 18), (4, 12), (4, 18), (8, 12), (8, 18)):
         gauges[(prec, recon)] = tm.device_buffer(tm.tm_gauge_bytes(L, prec, recon))
         tm.tm_gauge_pack(L, U, prec, recon, gauges[(prec, recon)], 1e-10)
     del U
@@ -166,6 +166,9 @@ def run_b200(args, rank, world, local_rank):
     codes_host = [torch.from_numpy(np.stack([ti.z4_codes(DIMS, seed=ti.NOISE_SEED + (rank * nb + b) * NRHS + r) for r in range(NRHS)]))
                   .pin_memory() for b in range(nb)]
     codes_dev = [c.cuda() for c in codes_host]
+    # the e2e leg ships the same noise bit-packed (3 bytes per site instead of 12: tm_tsm_batch_host_bits)
+    bits_host = [torch.from_numpy(np.stack([ti.z4_bits(DIMS, seed=ti.NOISE_SEED + (rank * nb + b) * NRHS + r) for r in range(NRHS)]))
+                 .pin_memory() for b in range(nb)]
     prec, recon = 2, 12
     g_lp = gauges[(prec, recon)]
     fb = tm.tm_spinor_bytes(L, prec, 1, NRHS)
@@ -188,7 +191,7 @@ def run_b200(args, rank, world, local_rank):
         iters_log.append([x.iters for x in info])
 
     def step_e2e(i):
-        rc, info = tm.tm_tsm_batch_host(L, g_lp, prec, recon, codes_host[i % nb], prm, NRHS, loops_host, tsm_ws)
+        rc, info = tm.tm_tsm_batch_host_bits(L, g_lp, prec, recon, bits_host[i % nb], prm, NRHS, loops_host, tsm_ws)
         assert rc == tm.TM_OK, rc
 
     def barrier():
@@ -223,12 +226,12 @@ def run_b200(args, rank, world, local_rank):
     ms_step = max_over_ranks(ms_step)
     value = world * NRHS / (ms_step * 1e-3)
 
-    # ---- e2e: host buffers through tm_tsm_batch_host, H2D + D2H inside the timed region ----
+    # ---- e2e: host buffers through tm_tsm_batch_host_bits, H2D + D2H inside the timed region ----
     for i in range(max(1, args.warmup // 2)):
         step_e2e(i)
     barrier()
     ms_e2e = max_over_ranks(time_events(torch, step_e2e, args.steps))
-    e2e = {"value": world * NRHS / (ms_e2e * 1e-3), "unit": "solves/s", "h2d_bytes_per_step": int(codes_host[0].numel()),
+    e2e = {"value": world * NRHS / (ms_e2e * 1e-3), "unit": "solves/s", "h2d_bytes_per_step": int(bits_host[0].numel()),
            "d2h_bytes_per_step": int(loops_host.numel() * 8), "ms_per_step": ms_e2e}
 
     # ---- roofline of the dominant kernel: the 12-RHS fp16 dslash launches inside the timed steps ----
@@ -282,7 +285,7 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
     kappa, mu = ti.KAPPA, ti.MU
     psi = torch.from_numpy(ti.z4(DIMS, seed=777).view(np.float64)).cuda()
     table = {}
-    for prec in (4, 2):
+    for prec in (8, 4, 2):  # double / single / half of Table A.1
         pb = tm.tm_spinor_bytes(L, prec, 0, 1)
         src = tm.device_buffer(2 * pb)
         tm.tm_spinor_pack(L, psi, prec, 1, src)
@@ -294,7 +297,9 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
         tmp = tm.device_buffer(2 * pb)
         for recon in (18, 12):
             g = gauges[(prec, recon)]
-            for kind, name, fl in ((tm.TM_KIND_TWIST_INV, "twist_inv", FLOPS_TWIST_INV), (tm.TM_KIND_XPAY_TWIST, "xpay_twist", FLOPS_XPAY)):
+            # "wilson_plain" = the hop alone (Table A.1's Wilson column: no twist in the epilogue)
+            for kind, name, fl in ((tm.TM_KIND_TWIST_INV, "twist_inv", FLOPS_TWIST_INV), (tm.TM_KIND_XPAY_TWIST, "xpay_twist", FLOPS_XPAY),
+                                   (tm.TM_KIND_PLAIN, "wilson_plain", 1320)):
                 def run(i, kind=kind, g=g, prec=prec, recon=recon):
                     tm.tm_dslash(L, g, prec, recon, bufs[i % 4], src[pb:2 * pb], xs[i % 4] if kind == tm.TM_KIND_XPAY_TWIST else None, 0, 0,
                                  kind, kappa, mu)

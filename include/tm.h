@@ -85,6 +85,9 @@ int tm_spinor_unpack(const tm_lattice* L, const void* packed, int prec, int nrhs
 /* Z2 x iZ2 noise from 2-bit codes: codes DEVICE uint8 [nrhs][V][12], bit0 = re<0, bit1 = im<0;
  * value = (+-1 +- i)/sqrt(2). */
 int tm_spinor_pack_z4(const tm_lattice* L, const unsigned char* codes, int prec, int nrhs, void* packed_out, void* stream);
+/* The same noise from bit-packed codes: codes3 DEVICE uint8 [nrhs][V][3]; the 24 bits of a site, little endian, hold component
+ * k = spin*3 + colour in bits 2k (re < 0) and 2k+1 (im < 0): 3 bytes per site instead of 12 on the host->device path. */
+int tm_spinor_pack_z4_bits(const tm_lattice* L, const unsigned char* codes3, int prec, int nrhs, void* packed_out, void* stream);
 
 /* ---- a2+a3: hopping term with fused local epilogue ("fused CUDA kernels, such as R_oo^-1 Dslash_oe,
  *      (R_ee - kappa^2 Dslash_eo) (and their daggered analogues)") ----------------------------------------- */
@@ -235,6 +238,12 @@ size_t tm_tsm_workspace_bytes(const tm_lattice* L, int prec_lp, int nrhs);
 int tm_tsm_batch_host(const tm_lattice* L, const void* gauge_lp, int prec_lp, int recon, const unsigned char* codes_host,
                       const tm_cg_params* p, int nrhs, tm_cg_info* info, double* loops_host, void* workspace,
                       size_t workspace_bytes, void* stream);
+
+/* The same with bit-packed noise codes (tm_spinor_pack_z4_bits): codes3_host HOST uint8 [nrhs][V][3], a quarter of the bytes
+ * over PCIe; identical results. */
+int tm_tsm_batch_host_bits(const tm_lattice* L, const void* gauge_lp, int prec_lp, int recon, const unsigned char* codes3_host,
+                           const tm_cg_params* p, int nrhs, tm_cg_info* info, double* loops_host, void* workspace,
+                           size_t workspace_bytes, void* stream);
 
 /* ---- instrumentation ------------------------------------------------------------------------------------- */
 /* Number of kernels this library has launched since load (all entry points). */

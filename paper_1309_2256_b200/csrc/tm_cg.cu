@@ -512,9 +512,9 @@ extern "C" size_t tm_tsm_workspace_bytes(const tm_lattice* L, int prec_lp, int n
            loop_workspace_bytes(L->g, nrhs) + round256((size_t)nrhs * 16 * L->g.T * 2 * sizeof(double));
 }
 
-extern "C" int tm_tsm_batch_host(const tm_lattice* L, const void* gauge_lp, int prec_lp, int recon, const unsigned char* codes_host,
-                                 const tm_cg_params* p, int nrhs, tm_cg_info* info, double* loops_host, void* workspace,
-                                 size_t workspace_bytes, void* stream)
+static int tsm_batch_host(const tm_lattice* L, const void* gauge_lp, int prec_lp, int recon, const unsigned char* codes_host,
+                          int bytes_per_site, const tm_cg_params* p, int nrhs, tm_cg_info* info, double* loops_host, void* workspace,
+                          size_t workspace_bytes, void* stream)
 {
     if (!L || !gauge_lp || !codes_host || !p || !info || !loops_host || !workspace) return TM_ERR_ARG;
     if (!valid_prec(prec_lp) || !valid_recon(recon) || nrhs < 1 || nrhs > TM_MAX_NRHS) return TM_ERR_ARG;
@@ -533,8 +533,8 @@ extern "C" int tm_tsm_batch_host(const tm_lattice* L, const void* gauge_lp, int 
     const size_t lb = (size_t)nrhs * 16 * g.T * 2 * sizeof(double);
     double* loops = static_cast<double*>(cv.take(lb));
     if (!cv.ok()) return TM_ERR_LAYOUT;
-    TM_CUDA_CHECK(cudaMemcpyAsync(codes, codes_host, (size_t)L->V * 12 * nrhs, cudaMemcpyHostToDevice, st));
-    int rc = spinor_pack_any(g, L->V, prec_lp, 2, nullptr, nullptr, codes, eta, nrhs, st);
+    TM_CUDA_CHECK(cudaMemcpyAsync(codes, codes_host, (size_t)L->V * bytes_per_site * nrhs, cudaMemcpyHostToDevice, st));
+    int rc = spinor_pack_any(g, L->V, prec_lp, bytes_per_site == 3 ? 3 : 2, nullptr, nullptr, codes, eta, nrhs, st);
     if (rc != TM_OK) return rc;
     tm_cg_params q = *p;
     q.mode = TM_CG_LP_TRUNCATED;
@@ -544,4 +544,18 @@ extern "C" int tm_tsm_batch_host(const tm_lattice* L, const void* gauge_lp, int 
     TM_CUDA_CHECK(cudaMemcpyAsync(loops_host, loops, lb, cudaMemcpyDeviceToHost, st));
     TM_CUDA_CHECK(cudaStreamSynchronize(st));
     return rc_cg;
+}
+
+extern "C" int tm_tsm_batch_host(const tm_lattice* L, const void* gauge_lp, int prec_lp, int recon, const unsigned char* codes_host,
+                                 const tm_cg_params* p, int nrhs, tm_cg_info* info, double* loops_host, void* workspace,
+                                 size_t workspace_bytes, void* stream)
+{
+    return tsm_batch_host(L, gauge_lp, prec_lp, recon, codes_host, 12, p, nrhs, info, loops_host, workspace, workspace_bytes, stream);
+}
+
+extern "C" int tm_tsm_batch_host_bits(const tm_lattice* L, const void* gauge_lp, int prec_lp, int recon, const unsigned char* codes3_host,
+                                      const tm_cg_params* p, int nrhs, tm_cg_info* info, double* loops_host, void* workspace,
+                                      size_t workspace_bytes, void* stream)
+{
+    return tsm_batch_host(L, gauge_lp, prec_lp, recon, codes3_host, 3, p, nrhs, info, loops_host, workspace, workspace_bytes, stream);
 }

@@ -68,7 +68,8 @@ __global__ void gauge_pack_kernel(Geo g, const double* __restrict__ U, char* out
     store_reals<PREC>(out + (size_t)pm * link_block, g.Vh, cb, u, RECON);
 }
 
-template <int PREC, int MODE> // MODE 0: pack from fp64 canonical, 1: unpack to fp64 canonical, 2: pack from Z2xiZ2 codes
+template <int PREC, int MODE> // MODE 0: pack from fp64 canonical, 1: unpack to fp64 canonical, 2: pack from Z2xiZ2 codes (one byte
+                              // per component), 3: from bit-packed codes (3 bytes per site: component k in bits 2k, 2k+1)
 __global__ void spinor_pack_kernel(Geo g, const double* __restrict__ src, double* dst, const unsigned char* __restrict__ codes,
                                    char* packed, size_t parity_bytes, long long V)
 {
@@ -97,6 +98,15 @@ __global__ void spinor_pack_kernel(Geo g, const double* __restrict__ src, double
             v[2 * k + 1] = (c & 2u) ? -r : r;
         }
         store_spinor<PREC>(field, g.Vh, cb, v);
+    } else if (MODE == 3) {
+        const real r = (real)0.70710678118654752440;
+        const unsigned w = (unsigned)codes[site * 3] | ((unsigned)codes[site * 3 + 1] << 8) | ((unsigned)codes[site * 3 + 2] << 16);
+#pragma unroll
+        for (int k = 0; k < 12; ++k) {
+            v[2 * k] = ((w >> (2 * k)) & 1u) ? -r : r;
+            v[2 * k + 1] = ((w >> (2 * k + 1)) & 1u) ? -r : r;
+        }
+        store_spinor<PREC>(field, g.Vh, cb, v);
     } else {
         load_spinor<PREC>(field, g.Vh, cb, v);
 #pragma unroll
@@ -122,7 +132,8 @@ static int spinor_pack_t(const Geo& g, long long V, int mode, const double* src,
     const size_t pb = spinor_parity_bytes(g, PREC);
     if (mode == 0) spinor_pack_kernel<PREC, 0><<<grid, block, 0, st>>>(g, src, dst, codes, (char*)packed, pb, V);
     else if (mode == 1) spinor_pack_kernel<PREC, 1><<<grid, block, 0, st>>>(g, src, dst, codes, (char*)packed, pb, V);
-    else spinor_pack_kernel<PREC, 2><<<grid, block, 0, st>>>(g, src, dst, codes, (char*)packed, pb, V);
+    else if (mode == 2) spinor_pack_kernel<PREC, 2><<<grid, block, 0, st>>>(g, src, dst, codes, (char*)packed, pb, V);
+    else spinor_pack_kernel<PREC, 3><<<grid, block, 0, st>>>(g, src, dst, codes, (char*)packed, pb, V);
     TM_LAUNCH_CHECK("spinor_pack_kernel");
     return TM_OK;
 }
@@ -184,4 +195,11 @@ extern "C" int tm_spinor_pack_z4(const tm_lattice* L, const unsigned char* codes
     if (!L || !codes || !out || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
     if (!aligned256(codes) || !aligned256(out)) return TM_ERR_LAYOUT;
     return spinor_pack_any(L->g, L->V, prec, 2, nullptr, nullptr, codes, out, nrhs, (cudaStream_t)stream);
+}
+
+extern "C" int tm_spinor_pack_z4_bits(const tm_lattice* L, const unsigned char* codes3, int prec, int nrhs, void* out, void* stream)
+{
+    if (!L || !codes3 || !out || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
+    if (!aligned256(codes3) || !aligned256(out)) return TM_ERR_LAYOUT;
+    return spinor_pack_any(L->g, L->V, prec, 3, nullptr, nullptr, codes3, out, nrhs, (cudaStream_t)stream);
 }

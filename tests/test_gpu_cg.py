@@ -143,6 +143,15 @@ def test_tsm_batch_host_end_to_end():
         assert abs(info[r].iters - iref["iters"]) <= 2
         ref = oracle.loop(eta, s_ref)
         assert rel(got[r], ref) < 3e-2  # LP solution differs from the oracle's at the truncation level
+    # bit-packed noise (3 bytes per site over PCIe): identical field, identical loops
+    bits = np.stack([ti.z4_bits(dims, seed=300 + r) for r in range(nrhs)])
+    a, b = tm.device_buffer(tm.tm_spinor_bytes(F.L, prec, 1, nrhs)), tm.device_buffer(tm.tm_spinor_bytes(F.L, prec, 1, nrhs))
+    tm.tm_spinor_pack_z4(F.L, torch.from_numpy(codes).cuda(), prec, nrhs, a)
+    tm.tm_spinor_pack_z4_bits(F.L, torch.from_numpy(bits).cuda(), prec, nrhs, b)
+    assert torch.equal(a, b)
+    loops2 = torch.zeros_like(loops_host).pin_memory()
+    rc2, info2 = tm.tm_tsm_batch_host_bits(F.L, F.gauge(prec, recon), prec, recon, torch.from_numpy(bits).pin_memory(), prm, nrhs, loops2, ws)
+    assert rc2 == tm.TM_OK and torch.equal(loops2, loops_host)
 
 
 def test_full_dilution_exact_trace_4x4():

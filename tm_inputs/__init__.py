@@ -117,6 +117,21 @@ def z4_codes(dims, seed=NOISE_SEED, t0=None, t1=None):
     return out
 
 
+def z4_bits(dims, seed=NOISE_SEED, t0=None, t1=None):
+    """z4_codes() bit-packed: 3 bytes per site, component k = spin*3 + colour in bits 2k (re < 0), 2k+1 (im < 0), little endian.
+    Packaging only (the 4x smaller host->device format of tm_spinor_pack_z4_bits)."""
+    c = z4_codes(dims, seed=seed, t0=t0, t1=t1).astype(np.uint32)
+    flat = c.reshape(-1, 12)
+    w = np.zeros(flat.shape[0], dtype=np.uint32)
+    for k in range(12):
+        w |= (flat[:, k] & 3) << (2 * k)
+    out = np.empty((flat.shape[0], 3), dtype=np.uint8)
+    out[:, 0] = w & 0xFF
+    out[:, 1] = (w >> 8) & 0xFF
+    out[:, 2] = (w >> 16) & 0xFF
+    return out.reshape(c.shape[:-2] + (3,))
+
+
 def z4_sites(sites, seed=NOISE_SEED):
     sites = np.ascontiguousarray(sites, dtype=np.int64)
     out = np.empty((sites.size, 4, 3), dtype=np.complex128)
