@@ -394,6 +394,29 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
         cg["fp64+fp%d" % (plp * 8)] = {"status": rc, "iters": info.iters, "reliable_updates": info.reliable_updates,
                                        "true_resid": info.true_resid, "seconds": dt, "ms_per_iter": 1e3 * dt / max(1, info.iters)}
         del ws
+    # the same tolerance by batched defect correction (TM_CG_HP_DEFECT): 12 sources share every gauge load of the inner solves;
+    # stopping rule |eta - M s| <= 1e-8 |eta| on the full lattice
+    del eta8, s8
+    pb8n = tm.tm_spinor_bytes(L, 8, 1, NRHS)
+    etaN, sN = tm.device_buffer(pb8n), tm.device_buffer(pb8n)
+    c1 = tm.device_buffer(L.V * 12)
+    for r in range(NRHS):
+        c1.copy_(torch.from_numpy(ti.z4_codes(DIMS, seed=ti.NOISE_SEED + 900 + r).reshape(-1)))
+        tm.tm_spinor_pack_z4(L, c1, 8, 1, etaN[r * pb8:(r + 1) * pb8])
+    for plp in (4, 2):
+        ws = tm.device_buffer(tm.tm_cg_workspace_bytes(L, 8, plp, tm.TM_CG_HP_DEFECT, NRHS))
+        prm = tm.make_cg_params(kappa, mu, 1e-8, 5000, tm.TM_CG_HP_DEFECT, 0.0)
+        torch.cuda.synchronize()
+        t0 = time.time()
+        rc, info = tm.tm_cg_multi(L, gauges[(8, 12)], 8, gauges[(plp, 12)], plp, 12, sN, etaN, prm, NRHS, ws)
+        torch.cuda.synchronize()
+        dt = time.time() - t0
+        cg["defect_x12_fp64+fp%d" % (plp * 8)] = {"status": rc, "nrhs": NRHS, "inner_iters": max(x.iters for x in info),
+                                                 "cycles": max(x.reliable_updates for x in info),
+                                                 "true_resid_full_system": max(x.true_resid for x in info), "seconds": dt,
+                                                 "ms_per_solve": 1e3 * dt / NRHS, "HP_solves_per_s": NRHS / dt}
+        del ws
+    del etaN, sN, c1
     out["cg_mixed_1e-8"] = cg
     if world == 1:
         base, _ = cpu_oracle_sample()

@@ -41,7 +41,7 @@ typedef struct tm_lattice tm_lattice; /* opaque host-side geometry descriptor */
 typedef enum { TM_PREC_F64 = 8, TM_PREC_F32 = 4, TM_PREC_F16 = 2 } tm_prec;   /* storage bytes per real */
 typedef enum { TM_RECON_18 = 18, TM_RECON_12 = 12 } tm_recon;                /* reals stored per link */
 typedef enum { TM_KIND_PLAIN = 0, TM_KIND_TWIST_INV = 1, TM_KIND_XPAY_TWIST = 2 } tm_dslash_kind;
-typedef enum { TM_CG_HP_MIXED = 0, TM_CG_LP_TRUNCATED = 1 } tm_cg_mode;
+typedef enum { TM_CG_HP_MIXED = 0, TM_CG_LP_TRUNCATED = 1, TM_CG_HP_DEFECT = 2 } tm_cg_mode;
 
 typedef enum {
     TM_OK = 0,
@@ -115,7 +115,8 @@ typedef struct {
     double tol;            /* stop when |r_k| <= tol |b''| (iterated residual of the normal system); 0: run max_iter */
     int max_iter;
     int mode;              /* tm_cg_mode */
-    double reliable_delta; /* HP_MIXED: recompute the true residual in prec_hp when |r| drops by this factor (0 -> 0.1) */
+    double reliable_delta; /* HP_MIXED: recompute the true residual in prec_hp when |r| drops by this factor (0 -> 0.1);
+                              HP_DEFECT: relative tolerance of each inner truncated solve (0 -> 3e-3) */
     int check_every;       /* LP_TRUNCATED: > 0: the host synchronises and reads the convergence flags every this many iterations;
                               0: pipelined poll -- flags follow every iteration into pinned host memory, the host stays one
                               iteration ahead of the GPU and stops one iteration after the last rhs converged */
@@ -134,6 +135,10 @@ typedef struct {
 /* Solve M(kappa,mu) s = eta on the full lattice through the even-even Schur system, x0 = 0:
  *   b' = eta_e + kappa Dslash_eo R^-1 eta_o; b'' = M_pc^dag b'; CG on M_pc^dag M_pc; s_o = R^-1 (eta_o + kappa Dslash_oe s_e).
  * HP_MIXED: eta/s packed full-lattice at prec_hp; iterations in prec_lp with reliable updates in prec_hp.
+ * HP_DEFECT: eta/s packed at prec_hp; defect correction (the other mixed-precision scheme of DESIGN.md reading 10): cycles of a
+ *   BATCHED truncated solve of M e = r in prec_lp to relative tolerance `reliable_delta` (0 -> 3e-3), s += e and r = eta - M s
+ *   in prec_hp, until |eta - M s| <= tol |eta| on the FULL lattice for every right-hand side.  All right-hand sides share every
+ *   gauge load of the inner solves.  info: iters = inner iterations, reliable_updates = cycles, true_resid = |eta - M s|/|eta|.
  * LP_TRUNCATED: eta/s packed at prec_lp, everything in prec_lp storage (fp32 arithmetic, fp64 reductions), no correction;
  *   gauge_hp may be NULL.
  * info: HOST.  The call synchronises `stream` before returning.  nrhs right-hand sides share every gauge load;

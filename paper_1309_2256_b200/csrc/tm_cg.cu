@@ -461,6 +461,149 @@ int cg_hp_mixed(const Geo& g, const void* gauge_hp, int prec_hp, const void* gau
     return status;
 }
 
+// aux of context entry 2 rhs (+ the parity offset already applied to c.scal) = sum of the per-warp partials, fixed order
+__global__ void __launch_bounds__(BLAS_THREADS) dot_finalize_strided_kernel(const double* partial, int ngroups, BlasCtx c)
+{
+    const int rhs = blockIdx.x;
+    double v = 0.0;
+    const double* p = partial + (size_t)rhs * ngroups;
+    for (int g = threadIdx.x; g < ngroups; g += BLAS_THREADS) v += p[g];
+    const double tot = block_sum(v);
+    if (threadIdx.x == 0) c.scal[2 * rhs].aux = tot;
+}
+
+// ---- HP by defect correction, batched (TM_CG_HP_DEFECT) ---------------------------------------------------------------
+// The alternative SURVEY.md 8(c-2) reading 10 names: outer residual and solution in the HP precision, inner solves by the
+// BATCHED truncated LP solver (every gauge load shared by all right-hand sides), restarted each cycle:
+//     s = 0, r = eta;  repeat: e = LP-solve(M e = r) to relative tolerance `reliable_delta`;  s += e;  r = eta - M s (HP)
+// until |eta - M s| <= tol |eta| for every right-hand side (the residual of the FULL system, both parities).
+int full_operator(const Geo& g, const void* gauge, int prec, int recon, void* out_full, const void* in_full, double kappa, double mu,
+                  int dagger, int nrhs, cudaStream_t st);
+
+size_t cg_defect_workspace_bytes(const Geo& g, int prec_hp, int prec_lp, int nrhs)
+{
+    return ctx_bytes(2 * nrhs) + round256(2 * spinor_parity_bytes(g, prec_hp) * nrhs) + 2 * round256(2 * spinor_parity_bytes(g, prec_lp) * nrhs) +
+           cg_lp_workspace_bytes(g, prec_lp, nrhs) + 2 * dot_partial_bytes(g, nrhs) + round256(sizeof(double) * nrhs);
+}
+
+int cg_hp_defect(const Geo& g, const void* gauge_hp, int prec_hp, const void* gauge_lp, int prec_lp, int recon, void* s_full,
+                 const void* eta_full, const tm_cg_params* prm, int nrhs, tm_cg_info* info, void* ws, size_t ws_bytes, cudaStream_t st)
+{
+    const size_t pbh = spinor_parity_bytes(g, prec_hp), pbl = spinor_parity_bytes(g, prec_lp);
+    const int nv = 2 * nrhs; // full-lattice arrays [rhs][parity] seen as nv one-parity vectors
+    Carver cv(ws, ws_bytes);
+    BlasCtx c = carve_ctx(cv, nv);
+    void* R = cv.take(2 * pbh * nrhs);
+    void* r_lp = cv.take(2 * pbl * nrhs);
+    void* e_lp = cv.take(2 * pbl * nrhs);
+    const size_t lpb = cg_lp_workspace_bytes(g, prec_lp, nrhs);
+    void* lpws = cv.take(lpb);
+    double* dotp[2] = {static_cast<double*>(cv.take(dot_partial_bytes(g, nrhs))), static_cast<double*>(cv.take(dot_partial_bytes(g, nrhs)))};
+    double* ones = static_cast<double*>(cv.take(sizeof(double) * nrhs));
+    if (!cv.ok()) return TM_ERR_LAYOUT;
+    int rc;
+    {
+        const std::vector<double> one(nrhs, 1.0);
+        TM_CUDA_CHECK(cudaMemcpyAsync(ones, one.data(), sizeof(double) * nrhs, cudaMemcpyHostToDevice, st));
+        TM_CUDA_CHECK(cudaStreamSynchronize(st));
+    }
+    tm_cg_params zero = *prm;
+    if ((rc = init_ctx(c, &zero, nv, st)) != TM_OK) return rc;
+    std::vector<CgScal> h(nv);
+    auto read_aux = [&](std::vector<double>& out) -> int {
+        TM_CUDA_CHECK(cudaMemcpyAsync(h.data(), c.scal, sizeof(CgScal) * nv, cudaMemcpyDeviceToHost, st));
+        TM_CUDA_CHECK(cudaStreamSynchronize(st));
+        for (int q = 0; q < nrhs; ++q) out[q] = h[2 * q].aux + h[2 * q + 1].aux;
+        return TM_OK;
+    };
+    std::vector<double> b2(nrhs), r2(nrhs);
+    if ((rc = k_norm2<FIN_AUX>(g, prec_hp, V_(eta_full, pbh), c, nv, st)) != TM_OK) return rc;
+    if ((rc = read_aux(b2)) != TM_OK) return rc;
+    TM_CUDA_CHECK(cudaMemsetAsync(s_full, 0, 2 * pbh * nrhs, st));
+    TM_CUDA_CHECK(cudaMemcpyAsync(R, eta_full, 2 * pbh * nrhs, cudaMemcpyDeviceToDevice, st));
+    r2 = b2;
+    tm_cg_params inner = *prm;
+    inner.mode = TM_CG_LP_TRUNCATED;
+    inner.tol = (prm->reliable_delta > 0 && prm->reliable_delta < 1) ? prm->reliable_delta : 3e-3;
+    inner.skip_true_resid = 1;
+    inner.check_every = 0;
+    std::vector<tm_cg_info> iinfo(nrhs);
+    for (int q = 0; q < nrhs; ++q) {
+        info[q].iters = 0;
+        info[q].reliable_updates = 0;
+        info[q].status = TM_ERR_MAXITER;
+    }
+    int total = 0;
+    bool done = false;
+    auto converged = [&]() {
+        bool all = true;
+        for (int q = 0; q < nrhs; ++q) {
+            const bool ok = b2[q] == 0.0 || r2[q] <= prm->tol * prm->tol * b2[q];
+            if (ok && info[q].status == TM_ERR_MAXITER) info[q].status = TM_OK;
+            all = all && ok;
+        }
+        return all;
+    };
+    done = converged();
+    int worst = TM_OK;
+    for (int cycle = 0; !done && total < prm->max_iter && cycle < 64; ++cycle) {
+        inner.max_iter = prm->max_iter - total;
+        // the last cycle only has to close the remaining gap: relax the inner tolerance to 0.3 tol / (worst current residual)
+        double worst_rel = 0.0;
+        for (int q = 0; q < nrhs; ++q)
+            if (b2[q] > 0) worst_rel = std::max(worst_rel, std::sqrt(r2[q] / b2[q]));
+        const double base_tol = (prm->reliable_delta > 0 && prm->reliable_delta < 1) ? prm->reliable_delta : 3e-3;
+        inner.tol = worst_rel > 0 ? std::min(0.5, std::max(base_tol, 0.3 * prm->tol / worst_rel)) : base_tol;
+        if ((rc = k_convert(g, prec_lp, prec_hp, V_(r_lp, pbl), VecArg{nullptr, 0}, V_(R, pbh), nv, st)) != TM_OK) return rc;
+        rc = cg_lp_truncated(g, gauge_lp, prec_lp, recon, e_lp, r_lp, &inner, nrhs, iinfo.data(), lpws, lpb, st);
+        if (rc == TM_ERR_CUDA || rc == TM_ERR_LAYOUT) return rc;
+        if (rc == TM_ERR_BREAKDOWN) worst = rc;
+        int it = 0;
+        for (int q = 0; q < nrhs; ++q) {
+            if (info[q].status == TM_ERR_MAXITER) { // still being refined: count its inner iterations and this cycle
+                info[q].iters += iinfo[q].iters;
+                info[q].reliable_updates += 1;
+            }
+            it = iinfo[q].iters > it ? iinfo[q].iters : it;
+        }
+        total += it > 0 ? it : 1;
+        // s += e (HP += LP), then R = eta - M s in HP: the subtraction and |R|^2 ride on the epilogue of the two dslash launches
+        // (fused_axpy with coefficient 1, per-warp fp64 partials), so eta, M s and R are not streamed a second time
+        if ((rc = k_axpby<0>(g, prec_hp, prec_lp, V_(s_full, pbh), V_(e_lp, pbl), 1.0, 1.0, c, nv, st)) != TM_OK) return rc;
+        for (int parity = 0; parity < 2; ++parity) {
+            DslashParams dp;
+            dp.gauge = gauge_hp; dp.nrhs = nrhs; dp.active = nullptr; dp.dagger = 0;
+            dp.out = static_cast<char*>(R) + parity * pbh;
+            dp.in = static_cast<const char*>(s_full) + (1 - parity) * pbh;
+            dp.x = static_cast<const char*>(s_full) + parity * pbh;
+            dp.out_parity = parity;
+            dp.rhs_stride_out = dp.rhs_stride_in = dp.rhs_stride_x = 2 * pbh;
+            dp.pq[0] = 1.0; dp.pq[1] = 2.0 * prm->kappa * prm->mu; dp.pq[2] = -prm->kappa; dp.pq[3] = 0.0;
+            dp.axpy_y = static_cast<const char*>(eta_full) + parity * pbh;
+            dp.axpy_y_stride = 2 * pbh;
+            dp.axpy_coef = ones;
+            dp.axpy_coef_stride = sizeof(double);
+            dp.dot_partial = dotp[parity];
+            if ((rc = launch_dslash(g, prec_hp, recon, dp, st)) != TM_OK) return rc;
+            // vector index of (rhs q, parity) in the context is 2 q + parity: finalize with a strided view of the context
+            BlasCtx cp = c;
+            cp.scal = c.scal + parity;
+            cp.active = c.active + parity;
+            dot_finalize_strided_kernel<<<nrhs, BLAS_THREADS, 0, st>>>(dotp[parity], (g.Vh + 31) / 32, cp);
+            TM_LAUNCH_CHECK("dot_finalize_strided_kernel");
+        }
+        if ((rc = read_aux(r2)) != TM_OK) return rc;
+        done = converged();
+    }
+    for (int q = 0; q < nrhs; ++q) {
+        const double rel = b2[q] > 0 ? std::sqrt(r2[q] / b2[q]) : 0.0;
+        info[q].iterated_resid = rel;
+        info[q].true_resid = rel;
+        if (info[q].status != TM_OK && worst == TM_OK) worst = info[q].status;
+    }
+    return worst;
+}
+
 } // namespace tmk
 
 using namespace tmk;
@@ -470,6 +613,7 @@ extern "C" size_t tm_cg_workspace_bytes(const tm_lattice* L, int prec_hp, int pr
     if (!L || !valid_prec(prec_lp) || nrhs < 1 || nrhs > TM_MAX_NRHS) return 0;
     if (mode == TM_CG_LP_TRUNCATED) return cg_lp_workspace_bytes(L->g, prec_lp, nrhs);
     if (!valid_prec(prec_hp)) return 0;
+    if (mode == TM_CG_HP_DEFECT) return cg_defect_workspace_bytes(L->g, prec_hp, prec_lp, nrhs);
     return cg_hp_workspace_bytes(L->g, prec_hp, prec_lp);
 }
 
@@ -484,7 +628,9 @@ extern "C" int tm_cg_multi(const tm_lattice* L, const void* gauge_hp, int prec_h
     cudaStream_t st = (cudaStream_t)stream;
     if (p->mode == TM_CG_LP_TRUNCATED)
         return cg_lp_truncated(L->g, gauge_lp, prec_lp, recon, s_full, eta_full, p, nrhs, info, workspace, workspace_bytes, st);
-    if (p->mode != TM_CG_HP_MIXED || !gauge_hp || !valid_prec(prec_hp) || !aligned256(gauge_hp)) return TM_ERR_ARG;
+    if ((p->mode != TM_CG_HP_MIXED && p->mode != TM_CG_HP_DEFECT) || !gauge_hp || !valid_prec(prec_hp) || !aligned256(gauge_hp)) return TM_ERR_ARG;
+    if (p->mode == TM_CG_HP_DEFECT)
+        return cg_hp_defect(L->g, gauge_hp, prec_hp, gauge_lp, prec_lp, recon, s_full, eta_full, p, nrhs, info, workspace, workspace_bytes, st);
     // HP_MIXED: right-hand sides are solved one after the other (reliable-update decisions are per solve)
     const size_t fb = 2 * spinor_parity_bytes(L->g, prec_hp);
     int worst = TM_OK;

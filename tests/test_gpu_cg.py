@@ -181,3 +181,27 @@ def test_full_dilution_exact_trace_4x4():
         acc += out.cpu().numpy().view(np.complex128)[..., 0].sum(axis=0)
     assert np.abs(acc[:, :3]).max() < 1e-12
     assert rel(acc[:, t], ref[:, t]) < 1e-9
+
+
+@pytest.mark.parametrize("prec_lp,recon", [(2, 12), (4, 12), (4, 18)])
+def test_cg_hp_defect_batched(prec_lp, recon):
+    """TM_CG_HP_DEFECT: fp64 outer residual, batched truncated inner solves (reading 10, second scheme).  The stopping
+    rule is the FULL-system residual |eta - M s| <= tol |eta|, checked here with the oracle's unpreconditioned operator (P8)."""
+    dims = (8, 8, 8, 16)
+    F, U = fields(dims)
+    nrhs, tol = 3, 1e-9
+    eta = np.stack([ti.z4(dims, seed=400 + r) for r in range(nrhs)])
+    pe = F.pack(eta, 8)
+    s = F.zeros_full(8, nrhs)
+    ws = tm.device_buffer(tm.tm_cg_workspace_bytes(F.L, 8, prec_lp, tm.TM_CG_HP_DEFECT, nrhs))
+    prm = tm.make_cg_params(KAPPA, MU, tol, 2000, tm.TM_CG_HP_DEFECT, 0.0)
+    rc, info = tm.tm_cg_multi(F.L, F.gauge(8, recon), 8, F.gauge(prec_lp, recon), prec_lp, recon, s, pe, prm, nrhs, ws)
+    assert rc == tm.TM_OK
+    got = F.unpack(s, 8, nrhs=nrhs)
+    for r in range(nrhs):
+        assert info[r].status == tm.TM_OK and 0 < info[r].true_resid <= tol
+        res = np.linalg.norm((eta[r] - oracle.M(U, got[r], KAPPA, MU)).ravel()) / np.linalg.norm(eta[r].ravel())
+        assert res <= 1.05 * tol and abs(res - info[r].true_resid) <= 0.05 * tol
+        s_ref, iref = oracle.cg_solve(U, eta[r], KAPPA, MU, 1e-12, 4000)
+        assert rel(got[r], s_ref) < 20 * tol
+        assert 2 <= info[r].reliable_updates <= 8 and info[r].iters >= iref["iters"] // 3
