@@ -155,7 +155,7 @@ def run_b200(args, rank, world, local_rank):
     # ---- once per configuration: gauge field -> packed links (a0) ----
     U = torch.from_numpy(ti.gauge(DIMS).view(np.float64)).cuda()
     gauges = {}
-    for prec, recon in ((2, 12), (2, 18), (4, 12), (4, 18), (8, 12), (8, 18)):
+    for prec, recon in ((2, 12), (2, 18), (4, 12), (4, 18), (8, 12), (8, 18), (2, 8), (4, 8), (8, 8)):
         gauges[(prec, recon)] = tm.device_buffer(tm.tm_gauge_bytes(L, prec, recon))
         tm.tm_gauge_pack(L, U, prec, recon, gauges[(prec, recon)], 1e-10)
     del U
@@ -295,7 +295,7 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
         for b in bufs + xs:
             b.copy_(src[:pb])
         tmp = tm.device_buffer(2 * pb)
-        for recon in (18, 12):
+        for recon in (18, 12, 8):  # 8 = the paper's fastest reconstruction on the GTX Titan (Table A.1); ALU-bound on B200
             g = gauges[(prec, recon)]
             # "wilson_plain" = the hop alone (Table A.1's Wilson column: no twist in the epilogue)
             for kind, name, fl in ((tm.TM_KIND_TWIST_INV, "twist_inv", FLOPS_TWIST_INV), (tm.TM_KIND_XPAY_TWIST, "xpay_twist", FLOPS_XPAY),

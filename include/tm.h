@@ -39,7 +39,7 @@ extern "C" {
 typedef struct tm_lattice tm_lattice; /* opaque host-side geometry descriptor */
 
 typedef enum { TM_PREC_F64 = 8, TM_PREC_F32 = 4, TM_PREC_F16 = 2 } tm_prec;   /* storage bytes per real */
-typedef enum { TM_RECON_18 = 18, TM_RECON_12 = 12 } tm_recon;                /* reals stored per link */
+typedef enum { TM_RECON_18 = 18, TM_RECON_12 = 12, TM_RECON_8 = 8 } tm_recon; /* reals stored per link */
 typedef enum { TM_KIND_PLAIN = 0, TM_KIND_TWIST_INV = 1, TM_KIND_XPAY_TWIST = 2 } tm_dslash_kind;
 typedef enum { TM_CG_HP_MIXED = 0, TM_CG_LP_TRUNCATED = 1, TM_CG_HP_DEFECT = 2 } tm_cg_mode;
 
@@ -50,7 +50,8 @@ typedef enum {
     TM_ERR_NOT_SU3 = -3,   /* tm_gauge_pack with recon 12: a link is farther than su3_tol from SU(3) */
     TM_ERR_CUDA = -4,      /* CUDA runtime error (no device, launch failure); tm_last_cuda_error() has the text */
     TM_ERR_BREAKDOWN = -5, /* CG: <p,Ap> <= 0 or NaN */
-    TM_ERR_MAXITER = -6    /* CG: max_iter reached before tol (solution still returned) */
+    TM_ERR_MAXITER = -6,   /* CG: max_iter reached before tol (solution still returned) */
+    TM_ERR_RECON8 = -7     /* tm_gauge_pack with recon 8: a link has |U01|^2 + |U02|^2 < 1e-6, where the 8-real chart is singular */
 } tm_status;
 
 #define TM_MAX_NRHS 16
@@ -73,7 +74,11 @@ size_t tm_spinor_bytes(const tm_lattice* L, int prec, int full, int nrhs);
 /* U_canonical: DEVICE, fp64 canonical, 4*V*18 doubles.  packed_out: DEVICE, tm_gauge_bytes().
  * recon 12 keeps rows 0,1 (row 2 = conj(row0 x row1) is rebuilt in the kernels; the antiperiodic sign is NOT
  * folded into stored links).  With recon 12, returns TM_ERR_NOT_SU3 if max |U U^dag - 1|, |row2 - conj(r0 x r1)|
- * exceeds su3_tol (this check synchronises the stream); su3_tol <= 0 skips the check. */
+ * exceeds su3_tol (this check synchronises the stream); su3_tol <= 0 skips the check.
+ * recon 8 ("8-parameter reconstruction"): U01, U02, U10 and arg(U00)/pi, arg(U20)/pi are stored; the kernels rebuild
+ * the link from unitarity (two square roots, two sincospi, one reciprocal of r = |U01|^2 + |U02|^2: errors grow like 1/r, so
+ * links with U00 of modulus ~1 lose accuracy; reading 31).  Same SU(3) check as recon 12; a field with a link of
+ * r < 1e-6 (the unit link has r = 0) is refused with TM_ERR_RECON8 (this check always synchronises the stream). */
 int tm_gauge_pack(const tm_lattice* L, const double* U_canonical, int prec, int recon, void* packed_out,
                   double su3_tol, void* stream);
 

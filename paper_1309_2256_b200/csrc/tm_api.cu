@@ -68,16 +68,16 @@ size_t link_cache_bytes(const Geo& g, int prec)
 
 int link_cache_build(const Geo& g, int prec, int recon, const void* gauge, void* cache, cudaStream_t st)
 {
-    if (prec == 4) return recon == 18 ? link_cache_build_t<4, 18>(g, gauge, cache, st) : link_cache_build_t<4, 12>(g, gauge, cache, st);
-    if (prec == 2) return recon == 18 ? link_cache_build_t<2, 18>(g, gauge, cache, st) : link_cache_build_t<2, 12>(g, gauge, cache, st);
+    if (prec == 4) return recon == 18 ? link_cache_build_t<4, 18>(g, gauge, cache, st) : recon == 12 ? link_cache_build_t<4, 12>(g, gauge, cache, st) : link_cache_build_t<4, 8>(g, gauge, cache, st);
+    if (prec == 2) return recon == 18 ? link_cache_build_t<2, 18>(g, gauge, cache, st) : recon == 12 ? link_cache_build_t<2, 12>(g, gauge, cache, st) : link_cache_build_t<2, 8>(g, gauge, cache, st);
     return TM_ERR_ARG;
 }
 
 int launch_dslash(const Geo& g, int prec, int recon, const DslashParams& p, cudaStream_t st)
 {
-    if (prec == 8) return recon == 18 ? launch_dslash_t<8, 18>(g, p, st) : launch_dslash_t<8, 12>(g, p, st);
-    if (prec == 4) return recon == 18 ? launch_dslash_t<4, 18>(g, p, st) : launch_dslash_t<4, 12>(g, p, st);
-    return recon == 18 ? launch_dslash_t<2, 18>(g, p, st) : launch_dslash_t<2, 12>(g, p, st);
+    if (prec == 8) return recon == 18 ? launch_dslash_t<8, 18>(g, p, st) : recon == 12 ? launch_dslash_t<8, 12>(g, p, st) : launch_dslash_t<8, 8>(g, p, st);
+    if (prec == 4) return recon == 18 ? launch_dslash_t<4, 18>(g, p, st) : recon == 12 ? launch_dslash_t<4, 12>(g, p, st) : launch_dslash_t<4, 8>(g, p, st);
+    return recon == 18 ? launch_dslash_t<2, 18>(g, p, st) : recon == 12 ? launch_dslash_t<2, 12>(g, p, st) : launch_dslash_t<2, 8>(g, p, st);
 }
 
 } // namespace tmk
@@ -92,7 +92,8 @@ extern "C" const char* tm_strerror(int s)
     case TM_OK: return "ok";
     case TM_ERR_ARG: return "invalid argument";
     case TM_ERR_LAYOUT: return "bad lattice dimensions, alignment or workspace size";
-    case TM_ERR_NOT_SU3: return "gauge link is not SU(3) within su3_tol (required for 12-real storage)";
+    case TM_ERR_NOT_SU3: return "gauge link is not SU(3) within su3_tol (required for 12- and 8-real storage)";
+    case TM_ERR_RECON8: return "a gauge link lies where the 8-real parametrisation is singular (|U01|^2 + |U02|^2 < 1e-6)";
     case TM_ERR_CUDA: return "CUDA runtime error (see tm_last_cuda_error)";
     case TM_ERR_BREAKDOWN: return "CG breakdown (<p,Ap> <= 0 or NaN)";
     case TM_ERR_MAXITER: return "CG reached max_iter before the requested tolerance";

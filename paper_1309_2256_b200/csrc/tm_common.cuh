@@ -70,7 +70,7 @@ static inline size_t spinor_parity_bytes(const Geo& g, int prec) { return (size_
 static inline size_t link_block_bytes(const Geo& g, int prec, int recon) { return (size_t)g.Vh * recon * prec; }
 
 static inline bool valid_prec(int p) { return p == 8 || p == 4 || p == 2; }
-static inline bool valid_recon(int r) { return r == 18 || r == 12; }
+static inline bool valid_recon(int r) { return r == 18 || r == 12 || r == 8; }
 
 // ---- internal launchers (defined in their own .cu files) ----
 struct DslashParams {

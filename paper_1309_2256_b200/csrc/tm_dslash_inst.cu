@@ -62,7 +62,11 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
         else if (n <= 6) launch_tile<TM_PREC, TM_RECON, 32, 6, 4, 1, false>(a, dg, st);
         else if (a.link_cache) {
             static const int tpc = getenv("TM_DSLASH_TPC") ? atoi(getenv("TM_DSLASH_TPC")) : 4;
-            if (tpc == 2) launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 2>(a, dg, st);
+            static const int lcv = getenv("TM_DSLASH_LC") ? atoi(getenv("TM_DSLASH_LC")) : 0;
+            if (lcv == 1) launch_tile_lc<TM_PREC, TM_RECON, 6, 5, 4>(a, dg, st);
+            else if (lcv == 2) launch_tile_lc<TM_PREC, TM_RECON, 4, 8, 4>(a, dg, st);
+            else if (lcv == 3) launch_tile_lc<TM_PREC, TM_RECON, 6, 4, 4>(a, dg, st);
+            else if (tpc == 2) launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 2>(a, dg, st);
             else if (tpc == 8) launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 8>(a, dg, st);
             else launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 4>(a, dg, st);
         }

@@ -441,9 +441,10 @@ extern "C" int tm_covdev(const tm_lattice* L, const void* gauge, int prec, int r
     if (!aligned256(gauge) || !aligned256(out_full) || !aligned256(in_full)) return TM_ERR_LAYOUT;
     cudaStream_t st = (cudaStream_t)stream;
     const Geo& g = L->g;
-    if (prec == 8) return recon == 18 ? covdev_launch<8, 18>(g, gauge, out_full, in_full, mu, nrhs, st) : covdev_launch<8, 12>(g, gauge, out_full, in_full, mu, nrhs, st);
-    if (prec == 4) return recon == 18 ? covdev_launch<4, 18>(g, gauge, out_full, in_full, mu, nrhs, st) : covdev_launch<4, 12>(g, gauge, out_full, in_full, mu, nrhs, st);
-    return recon == 18 ? covdev_launch<2, 18>(g, gauge, out_full, in_full, mu, nrhs, st) : covdev_launch<2, 12>(g, gauge, out_full, in_full, mu, nrhs, st);
+#define TM_COVDEV(P) (recon == 18 ? covdev_launch<P, 18>(g, gauge, out_full, in_full, mu, nrhs, st) : recon == 12 ? covdev_launch<P, 12>(g, gauge, out_full, in_full, mu, nrhs, st) : covdev_launch<P, 8>(g, gauge, out_full, in_full, mu, nrhs, st))
+    if (prec == 8) return TM_COVDEV(8);
+    if (prec == 4) return TM_COVDEV(4);
+    return TM_COVDEV(2);
 }
 
 extern "C" int tm_contract_field(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, double* out,

@@ -12,7 +12,9 @@
 //   fp32: 18 -> 4 float4 chunks + 1 float2 tail array; 12 -> 3 float4 chunks
 //   fp16: 18 -> 2 uint4 chunks + 1 half2 (4-byte) tail array; 12 -> 1 uint4 chunk + 1 uint2 (8-byte) tail array
 // Links are stored unscaled (|U_ij| <= 1).  With R = 12 the third row is rebuilt as conj(row0 x row1)
-// ("12-parameter reconstruction").
+// ("12-parameter reconstruction").  R = 8 ("8-parameter reconstruction ... only the coefficients
+// are stored (8 real numbers)"; the paper gives no formulas, reading 31): U01, U02, U10 and the phases of U00 and U20
+// in units of pi; fp64: 4 double2 chunks, fp32: 2 float4, fp16: 1 uint4.  rebuild_from8() below.
 #pragma once
 #include "tm_common.cuh"
 
@@ -129,10 +131,63 @@ __device__ __forceinline__ void rebuild_row2(real* u)
     }
 }
 
+// 8 stored reals q = (U01, U02, U10, arg U00 / pi, arg U20 / pi) -> u[18].  Unitarity of row 0 and column 0 gives |U00|, |U20|;
+// row 1 follows from  row1 . conj(row0) = 0  and  (row0 x row1)_0 = conj(U20)  (two linear equations in U11, U12 with determinant
+// r = |U01|^2 + |U02|^2), row 2 = conj(row0 x row1).  Ill-conditioned as r -> 0 (errors grow like 1/r).
+template <typename real>
+__device__ __forceinline__ void rebuild_from8(const real* q, real* u)
+{
+    const real a1r = q[0], a1i = q[1], a2r = q[2], a2i = q[3], br = q[4], bi = q[5];
+    const real r = a1r * a1r + a1i * a1i + a2r * a2r + a2i * a2i;
+    const real m00 = sqrt(fmax(real(0), real(1) - r));
+    real s0, c0, s1, c1;
+    sincospi(q[6], &s0, &c0);
+    sincospi(q[7], &s1, &c1);
+    const real u00r = m00 * c0, u00i = m00 * s0;
+    const real m20 = sqrt(fmax(real(0), r - br * br - bi * bi));
+    const real u20r = m20 * c1, u20i = m20 * s1;
+    const real rinv = real(1) / r;
+    // t = U10 conj(U00)
+    const real tr = br * u00r + bi * u00i, ti = bi * u00r - br * u00i;
+    // U11 = -(t U01 + conj(U02) conj(U20)) / r ; conj(U02) conj(U20) = conj(U02 U20)
+    const real pr = a2r * u20r - a2i * u20i, pi_ = a2r * u20i + a2i * u20r; // U02 U20
+    const real u11r = -(tr * a1r - ti * a1i + pr) * rinv, u11i = -(tr * a1i + ti * a1r - pi_) * rinv;
+    // U12 = (conj(U01 U20) - t U02) / r
+    const real wr = a1r * u20r - a1i * u20i, wi = a1r * u20i + a1i * u20r; // U01 U20
+    const real u12r = (wr - (tr * a2r - ti * a2i)) * rinv, u12i = (-wi - (tr * a2i + ti * a2r)) * rinv;
+    u[0] = u00r; u[1] = u00i; u[2] = a1r; u[3] = a1i; u[4] = a2r; u[5] = a2i;
+    u[6] = br; u[7] = bi; u[8] = u11r; u[9] = u11i; u[10] = u12r; u[11] = u12i;
+    rebuild_row2(u);
+}
+
 template <int PREC, int RECON>
 __device__ __forceinline__ void load_link(const void* block, int Vh, int cb, typename Prec<PREC>::real* u)
 {
-    if constexpr (PREC == 8) {
+    if constexpr (RECON == 8) {
+        typename Prec<PREC>::real q[8];
+        if constexpr (PREC == 8) {
+            const double2* p = reinterpret_cast<const double2*>(block) + cb;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const double2 d = __ldg(p + (size_t)k * Vh);
+                q[2 * k] = d.x;
+                q[2 * k + 1] = d.y;
+            }
+        } else if constexpr (PREC == 4) {
+            const float4* p = reinterpret_cast<const float4*>(block) + cb;
+            const float4 d0 = __ldg(p), d1 = __ldg(p + (size_t)Vh);
+            q[0] = d0.x; q[1] = d0.y; q[2] = d0.z; q[3] = d0.w;
+            q[4] = d1.x; q[5] = d1.y; q[6] = d1.z; q[7] = d1.w;
+        } else {
+            const uint4 d = __ldg(reinterpret_cast<const uint4*>(block) + cb);
+            unpack_h2(d.x, q[0], q[1]);
+            unpack_h2(d.y, q[2], q[3]);
+            unpack_h2(d.z, q[4], q[5]);
+            unpack_h2(d.w, q[6], q[7]);
+        }
+        rebuild_from8(q, u);
+        return;
+    } else if constexpr (PREC == 8) {
         const double2* p = reinterpret_cast<const double2*>(block) + cb;
 #pragma unroll
         for (int k = 0; k < RECON / 2; ++k) {

@@ -4,6 +4,7 @@
 namespace tmk {
 
 __device__ unsigned int g_su3_dev_bits; // max deviation from SU(3) seen by the last gauge pack (float bits)
+__device__ unsigned int g_r8_inv_bits;  // recon 8: max 1 / (|U01|^2 + |U02|^2) seen by the last gauge pack (float bits)
 
 template <int PREC>
 __device__ __forceinline__ void store_reals(void* block, int Vh, int cb, const double* u, int n)
@@ -65,6 +66,13 @@ __global__ void gauge_pack_kernel(Geo g, const double* __restrict__ U, char* out
         if (!(dev == dev)) dev = 1e30; // NaN
         atomicMax(&g_su3_dev_bits, __float_as_uint((float)dev));
     }
+    if (RECON == 8) { // U01, U02, U10, arg(U00)/pi, arg(U20)/pi (tm_layout.cuh rebuild_from8)
+        const double r8 = u[2] * u[2] + u[3] * u[3] + u[4] * u[4] + u[5] * u[5];
+        atomicMax(&g_r8_inv_bits, __float_as_uint(r8 > 1e-30 ? (float)fmin(1.0 / r8, 1e30) : 1e30f));
+        double q[8] = {u[2], u[3], u[4], u[5], u[6], u[7], atan2(u[1], u[0]) / 3.14159265358979323846, atan2(u[13], u[12]) / 3.14159265358979323846};
+        store_reals<PREC>(out + (size_t)pm * link_block, g.Vh, cb, q, 8);
+        return;
+    }
     store_reals<PREC>(out + (size_t)pm * link_block, g.Vh, cb, u, RECON);
 }
 
@@ -119,6 +127,7 @@ static int gauge_pack_t(const Geo& g, const double* U, int recon, void* out, int
 {
     dim3 block(128), grid((g.Vh + 127) / 128, 8);
     if (recon == 18) gauge_pack_kernel<PREC, 18><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 18), check);
+    else if (recon == 8) gauge_pack_kernel<PREC, 8><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 8), check);
     else gauge_pack_kernel<PREC, 12><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 12), check);
     TM_LAUNCH_CHECK("gauge_pack_kernel");
     return TM_OK;
@@ -155,10 +164,14 @@ extern "C" int tm_gauge_pack(const tm_lattice* L, const double* U, int prec, int
     if (!L || !U || !out || !valid_prec(prec) || !valid_recon(recon)) return TM_ERR_ARG;
     if (!aligned256(U) || !aligned256(out)) return TM_ERR_LAYOUT;
     cudaStream_t st = (cudaStream_t)stream;
-    const int check = (recon == 12 && su3_tol > 0) ? 1 : 0;
+    const int check = (recon != 18 && su3_tol > 0) ? 1 : 0;
     if (check) {
         const unsigned int zero = 0;
         TM_CUDA_CHECK(cudaMemcpyToSymbolAsync(g_su3_dev_bits, &zero, sizeof(zero), 0, cudaMemcpyHostToDevice, st));
+    }
+    if (recon == 8) {
+        const unsigned int zero = 0;
+        TM_CUDA_CHECK(cudaMemcpyToSymbolAsync(g_r8_inv_bits, &zero, sizeof(zero), 0, cudaMemcpyHostToDevice, st));
     }
     int rc;
     if (prec == 8) rc = gauge_pack_t<8>(L->g, U, recon, out, check, st);
@@ -172,6 +185,14 @@ extern "C" int tm_gauge_pack(const tm_lattice* L, const double* U, int prec, int
         float dev;
         memcpy(&dev, &bits, sizeof(dev));
         if (dev > su3_tol) return TM_ERR_NOT_SU3;
+    }
+    if (recon == 8) { // the 8-real chart is singular where U01 = U02 = 0 (e.g. the unit link): refuse such fields
+        unsigned int bits = 0;
+        TM_CUDA_CHECK(cudaMemcpyFromSymbolAsync(&bits, g_r8_inv_bits, sizeof(bits), 0, cudaMemcpyDeviceToHost, st));
+        TM_CUDA_CHECK(cudaStreamSynchronize(st));
+        float rinv;
+        memcpy(&rinv, &bits, sizeof(rinv));
+        if (rinv > 1e6f) return TM_ERR_RECON8;
     }
     return TM_OK;
 }

@@ -71,7 +71,7 @@ def test_cg_hp_mixed(prec_lp, recon):
     assert info[0].iters <= (2 if prec_lp == 4 else 4) * iref["iters"] + 10
 
 
-@pytest.mark.parametrize("prec,recon", [(2, 12), (2, 18), (4, 12)])
+@pytest.mark.parametrize("prec,recon", [(2, 12), (2, 18), (4, 12), (2, 8), (4, 8)])
 def test_cg_lp_truncated_batched(prec, recon):
     """configs[3] in small: 12 truncated solves (tol 1e-2) sharing every gauge load; batched == unbatched bit for bit."""
     dims = (8, 8, 8, 16)

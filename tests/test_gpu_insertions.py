@@ -26,7 +26,7 @@ def cplx(t):
     return t.cpu().numpy().view(np.complex128)[..., 0]
 
 
-@pytest.mark.parametrize("prec,recon", [(8, 18), (8, 12), (4, 18), (4, 12), (2, 12), (2, 18)])
+@pytest.mark.parametrize("prec,recon", [(8, 18), (8, 12), (4, 18), (4, 12), (2, 12), (2, 18), (8, 8), (4, 8), (2, 8)])
 def test_covdev(prec, recon):
     """D_mu on an antiperiodic lattice with four different extents (every wrap-around, the temporal sign), 2 right-hand sides."""
     dims = (4, 6, 8, 10)

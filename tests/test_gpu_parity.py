@@ -111,7 +111,7 @@ def run_dslash(F, prec, recon, psi, x, out_parity, dagger, kind):
 
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 6, 8, 10), (8, 4, 6, 4)])
 @pytest.mark.parametrize("prec", [8, 4, 2])
-@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("recon", [18, 12, 8])
 def test_dslash_all_kinds(dims, prec, recon):
     F, U = fields(dims)
     psi, x = ti.gauss_spinor(dims, 3), ti.gauss_spinor(dims, 4)
@@ -122,6 +122,23 @@ def test_dslash_all_kinds(dims, prec, recon):
                 ref = oracle_dslash(U, psi, x, out_parity, dagger, kind)
                 assert rel(got, ref) < TOL[prec], (dims, prec, recon, out_parity, dagger, kind)
                 assert not oracle.project(got, 1 - out_parity).any()
+
+
+def test_gauge_pack_recon8_refuses_the_singular_chart():
+    """The unit link has U01 = U02 = 0: the 8 stored reals do not determine it (reading 31)."""
+    dims = (4, 4, 4, 4)
+    L = tm.tm_lattice_create(dims)
+    buf = tm.device_buffer(tm.tm_gauge_bytes(L, 4, 8))
+    with pytest.raises(tm.TmError) as e:
+        tm.tm_gauge_pack(L, to_dev(ti.unit_gauge(dims)), 4, 8, buf, 1e-10)
+    assert e.value.status == tm.TM_ERR_RECON8
+    U = ti.gauge(dims).copy()
+    U[1, 2, 3, 0, 2, 1, 1] *= 1.01
+    with pytest.raises(tm.TmError) as e:
+        tm.tm_gauge_pack(L, to_dev(U), 4, 8, buf, 1e-10)
+    assert e.value.status == tm.TM_ERR_NOT_SU3
+    tm.tm_gauge_pack(L, to_dev(ti.gauge(dims)), 4, 8, buf, 1e-10)
+    assert tm.tm_gauge_bytes(L, 4, 8) * 18 == tm.tm_gauge_bytes(L, 4, 18) * 8
 
 
 @pytest.mark.parametrize("prec,recon", [(8, 18), (8, 12), (4, 12), (2, 12), (2, 18)])
@@ -163,7 +180,8 @@ def test_dslash_16x32_and_general_epilogue(prec):
     assert rel(F.unpack(out, prec), ref) < TOL[prec]
 
 
-@pytest.mark.parametrize("prec,recon,nrhs", [(8, 18, 2), (8, 12, 3), (4, 18, 12), (4, 12, 5), (2, 12, 12), (2, 18, 8), (2, 12, 16)])
+@pytest.mark.parametrize("prec,recon,nrhs", [(8, 18, 2), (8, 12, 3), (4, 18, 12), (4, 12, 5), (2, 12, 12), (2, 18, 8), (2, 12, 16), (4, 8, 12),
+                                             (2, 8, 5), (8, 8, 2)])
 def test_dslash_multi_rhs_equals_single(prec, recon, nrhs):
     dims = (4, 6, 8, 10)
     F, U = fields(dims)
@@ -185,7 +203,7 @@ def test_dslash_multi_rhs_equals_single(prec, recon, nrhs):
 # ---- a4: MdagM -------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("dims", [(4, 4, 4, 4), (4, 6, 8, 10)])
 @pytest.mark.parametrize("prec", [8, 4, 2])
-@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("recon", [18, 12, 8])
 def test_MdagM(dims, prec, recon):
     F, U = fields(dims)
     psi = ti.gauss_spinor(dims, 17)
