@@ -48,7 +48,7 @@ def test_lattice_and_sizes(tm):
     assert tm.tm_spinor_bytes(L, 2, 0, 1) == V // 2 * (24 * 2 + 4)
     assert tm.tm_spinor_bytes(L, 2, 1, 12) == 12 * V * (24 * 2 + 4)
     assert tm.tm_cg_workspace_bytes(L, 8, 2, tm.TM_CG_LP_TRUNCATED, 12) > 6 * 12 * tm.tm_spinor_bytes(L, 2, 0, 1)
-    assert tm.tm_gauge_bytes(L, 3, 18) == 0 and tm.tm_gauge_bytes(L, 4, 8) == 0
+    assert tm.tm_gauge_bytes(L, 3, 18) == 0 and tm.tm_gauge_bytes(L, 4, 9) == 0 and tm.tm_gauge_bytes(L, 4, 8) * 18 == tm.tm_gauge_bytes(L, 4, 18) * 8
 
 
 def test_no_cpu_fallback(tm):
