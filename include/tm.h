@@ -8,7 +8,8 @@
  *  - Plain C types only.  `stream` arguments are a cudaStream_t passed as void* (NULL = legacy default stream).
  *  - OWNERSHIP: the caller owns all device memory.  The library never allocates device memory; workspaces are
  *    passed in, sized by the tm_*_bytes() queries.  Pointers are borrowed until the stream work completes.
- *    Every device buffer must be 256-byte aligned.  "device" / "host" is stated per argument.
+ *    Every device buffer must be 256-byte aligned; the one-parity spinor arguments of tm_dslash* / tm_MdagM may also be the
+ *    even / odd block of a full-lattice buffer (16-byte alignment suffices there).  "device" / "host" is stated per argument.
  *  - ERRORS: every entry point returns int: TM_OK (0) or a negative tm_status.  No exceptions, no exit().
  *    Calls are asynchronous on `stream` unless they fill host structs (tm_cg*, tm_tsm_batch_host: documented).
  *  - There is no CPU fallback: without a CUDA device every compute call returns TM_ERR_CUDA.

@@ -169,7 +169,8 @@ static int dslash_common(const tm_lattice* L, const void* gauge, int prec, int r
     if (!L || !gauge || !out || !in || !valid_prec(prec) || !valid_recon(recon)) return TM_ERR_ARG;
     if (out == in || nrhs < 1 || nrhs > TM_MAX_NRHS || (out_parity & ~1)) return TM_ERR_ARG;
     if (!x && (pq[0] != 0.0 || pq[1] != 0.0)) return TM_ERR_ARG;
-    if (!aligned256(gauge) || !aligned256(out) || !aligned256(in) || (x && !aligned256(x))) return TM_ERR_LAYOUT;
+    // one-parity spinors may be views into a full-lattice buffer (odd block at + parity bytes): 16-byte chunks must stay aligned
+    if (!aligned256(gauge) || !aligned16(out) || !aligned16(in) || (x && !aligned16(x))) return TM_ERR_LAYOUT;
     DslashParams p;
     p.gauge = gauge; p.out = out; p.in = in;
     p.x = (pq[0] != 0.0 || pq[1] != 0.0) ? x : nullptr;
@@ -253,7 +254,7 @@ extern "C" int tm_MdagM(const tm_lattice* L, const void* gauge, int prec, int re
 {
     if (!L || !gauge || !out || !in || !tmp || !valid_prec(prec) || !valid_recon(recon)) return TM_ERR_ARG;
     if (nrhs < 1 || nrhs > TM_MAX_NRHS || (parity & ~1)) return TM_ERR_ARG;
-    if (!aligned256(gauge) || !aligned256(out) || !aligned256(in) || !aligned256(tmp)) return TM_ERR_LAYOUT;
+    if (!aligned256(gauge) || !aligned16(out) || !aligned16(in) || !aligned256(tmp)) return TM_ERR_LAYOUT;
     const size_t pb = spinor_parity_bytes(L->g, prec);
     return mdagm_apply(L->g, gauge, prec, recon, out, pb, in, pb, tmp, parity, kappa, mu, nrhs, nullptr, (cudaStream_t)stream);
 }

@@ -63,6 +63,7 @@ int cuda_fail(cudaError_t e, const char* where);
     } while (0)
 
 static inline bool aligned256(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 255u) == 0; }
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; } // one-parity views
 static inline size_t round256(size_t n) { return (n + 255) & ~size_t(255); }
 
 // bytes of one single-parity spinor / one (parity,mu) link block

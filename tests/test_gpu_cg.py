@@ -205,3 +205,31 @@ def test_cg_hp_defect_batched(prec_lp, recon):
         s_ref, iref = oracle.cg_solve(U, eta[r], KAPPA, MU, 1e-12, 4000)
         assert rel(got[r], s_ref) < 20 * tol
         assert 2 <= info[r].reliable_updates <= 8 and info[r].iters >= iref["iters"] // 3
+
+
+def test_cg_lp_truncated_ragged_6x6x6x6():
+    """Vh = 648: the last 32-site tile of the link-cache kernel holds 8 sites and the fp16 parity block (33 696 B) is not a
+    multiple of 256 B; 12 right-hand sides, iteration counts against the oracle CG, batched == unbatched bit for bit."""
+    dims = (6, 6, 6, 6)
+    F, U = fields(dims)
+    nrhs, prec, recon = 12, 2, 12
+    eta = np.stack([ti.z4(dims, seed=800 + r) for r in range(nrhs)])
+    pe = F.pack(eta, prec)
+    s = F.zeros_full(prec, nrhs)
+    ws = tm.device_buffer(tm.tm_cg_workspace_bytes(F.L, 8, prec, tm.TM_CG_LP_TRUNCATED, nrhs))
+    prm = tm.make_cg_params(KAPPA, MU, 1e-2, 500, tm.TM_CG_LP_TRUNCATED)
+    rc, info = tm.tm_cg_multi(F.L, None, 8, F.gauge(prec, recon), prec, recon, s, pe, prm, nrhs, ws)
+    assert rc == tm.TM_OK
+    got = F.unpack(s, prec, nrhs=nrhs)
+    for r in (0, 11):
+        s_ref, iref = oracle.cg_solve(U, eta[r], KAPPA, MU, 1e-2, 500)
+        assert abs(info[r].iters - iref["iters"]) <= 2
+        assert rel(got[r], s_ref) < 3e-2
+    s1 = F.zeros_full(prec, 1)
+    ws1 = tm.device_buffer(tm.tm_cg_workspace_bytes(F.L, 8, prec, tm.TM_CG_LP_TRUNCATED, 1))
+    fb = tm.tm_spinor_bytes(F.L, prec, 1, 1)
+    e1 = tm.device_buffer(fb)  # the slice of the batch is only 16-byte aligned on this lattice: copy to an aligned buffer
+    e1.copy_(pe[5 * fb:6 * fb])
+    rc1, info1 = tm.tm_cg(F.L, None, 8, F.gauge(prec, recon), prec, recon, s1, e1, prm, ws1)
+    assert rc1 == tm.TM_OK and info1.iters == info[5].iters
+    assert torch.equal(s1, s[5 * fb:6 * fb])

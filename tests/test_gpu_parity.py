@@ -242,3 +242,36 @@ def test_loop_contract(dims, prec):
     out2 = torch.zeros_like(out)
     tm.tm_loop_contract(F.L, pa, pa, prec, nrhs, out2, ws)
     assert torch.equal(out, out2)
+
+
+# ---- ragged tails: Vh = 648 is not a multiple of the 32-site tiles / 128-site CTAs, X/2 = 3 is odd -------------------
+@pytest.mark.parametrize("prec,recon", [(8, 12), (4, 18), (4, 12), (2, 12), (2, 8)])
+def test_ragged_lattice_6x6x6x6(prec, recon):
+    dims = (6, 6, 6, 6)
+    F, U = fields(dims)
+    nrhs = 12
+    psi = np.stack([ti.gauss_spinor(dims, 700 + r) for r in range(nrhs)])
+    x = np.stack([ti.z4(dims, seed=720 + r) for r in range(nrhs)])
+    # single rhs, every kind
+    for out_parity, dagger, kind in ((0, 0, 1), (1, 1, 2), (1, 0, 0)):
+        got = run_dslash(F, prec, recon, psi[0], x[0], out_parity, dagger, kind)
+        assert rel(got, oracle_dslash(U, psi[0], x[0], out_parity, dagger, kind)) < TOL[prec]
+    # 12 right-hand sides through the multi-rhs tile kernels (last tile has 8 of 32 sites)
+    pin, px = F.pack(psi, prec), F.pack(x, prec)
+    pb = F.pb(prec)
+    ostack = tm.device_buffer(pb * nrhs)
+    tm.tm_dslash(F.L, F.gauge(prec, recon), prec, recon, ostack, F.half(pin, prec, 1, nrhs), F.half(px, prec, 0, nrhs), 0, 0, 2, KAPPA, MU,
+                 nrhs)
+    full = F.zeros_full(prec, nrhs)
+    F.put_half(full, ostack, prec, 0, nrhs)
+    got = F.unpack(full, prec, nrhs=nrhs)
+    for r in (0, 5, 11):
+        assert rel(got[r], oracle_dslash(U, psi[r], x[r], 0, 0, 2)) < TOL[prec]
+    # loops of 3 right-hand sides
+    T = dims[3]
+    out = torch.zeros((nrhs, 16, T, 2), dtype=torch.float64, device="cuda")
+    ws = tm.device_buffer(tm.tm_loop_workspace_bytes(F.L, nrhs))
+    tm.tm_loop_contract(F.L, px, pin, prec, nrhs, out, ws)
+    got = out.cpu().numpy().view(np.complex128)[..., 0]
+    for r in (0, 7):
+        assert rel(got[r], oracle.loop(x[r], psi[r])) < TOL[prec]
