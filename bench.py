@@ -33,7 +33,7 @@ FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12          # 148 SMs x 128 FP32 
 
 
 # one `ncu --set full` capture of the dominant kernel (profiles/r01_ncu_dslash_fp16_recon12_12rhs.md), bytes per launch
-NCU_DRAM_BYTES_PER_LAUNCH = 2.6016e9
+NCU_DRAM_BYTES_PER_LAUNCH = 2.6145e9
 
 
 def peaks():
@@ -314,13 +314,13 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
                     "us": ms * 1e3, "GFLOPS": Vh * fl / ms / 1e6, "GBps_algorithmic": gbs, "GBps_naive_model": naive / ms / 1e6,
                     "bytes_per_site_minimal": by / Vh, "bytes_per_site_naive": naive / Vh,
                     "frac_of_measured_%.0f" % hbm_peak: gbs / hbm_peak, "frac_of_nominal_8000": gbs / 8000.0}
-            def run_mdagm(i, g=gauges[(prec, 12)], prec=prec):
-                tm.tm_MdagM(L, g, prec, 12, bufs[i % 4], src[:pb], tmp, 0, kappa, mu)
-            for i in range(3):
-                run_mdagm(i)
-            ms = min(time_events(torch, run_mdagm, 20) for _ in range(3))
-            table["MdagM_fp%d_recon12" % (prec * 8)] = {"us": ms * 1e3, "GFLOPS": Vh * 2 * (FLOPS_TWIST_INV + FLOPS_XPAY) / ms / 1e6,
-                                                       "GBps_algorithmic": (2 * dslash_bytes(Vh, prec, 12, False) + 2 * dslash_bytes(Vh, prec, 12, True)) / ms / 1e6}
+        def run_mdagm(i, g=gauges[(prec, 12)], prec=prec):
+            tm.tm_MdagM(L, g, prec, 12, bufs[i % 4], src[:pb], tmp, 0, kappa, mu)
+        for i in range(3):
+            run_mdagm(i)
+        ms = min(time_events(torch, run_mdagm, 20) for _ in range(3))
+        table["MdagM_fp%d_recon12" % (prec * 8)] = {"us": ms * 1e3, "GFLOPS": Vh * 2 * (FLOPS_TWIST_INV + FLOPS_XPAY) / ms / 1e6,
+                                                   "GBps_algorithmic": (2 * dslash_bytes(Vh, prec, 12, False) + 2 * dslash_bytes(Vh, prec, 12, True)) / ms / 1e6}
         del bufs, xs, src, tmp
     out["dslash"] = table
     out["dslash_peak_source"] = peak_src

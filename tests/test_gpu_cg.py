@@ -233,3 +233,24 @@ def test_cg_lp_truncated_ragged_6x6x6x6():
     rc1, info1 = tm.tm_cg(F.L, None, 8, F.gauge(prec, recon), prec, recon, s1, e1, prm, ws1)
     assert rc1 == tm.TM_OK and info1.iters == info[5].iters
     assert torch.equal(s1, s[5 * fb:6 * fb])
+
+
+def test_cg_breakdown_is_per_rhs():
+    """A NaN source makes <p,Ap> NaN: that right-hand side stops with TM_ERR_BREAKDOWN, the others of the batch converge."""
+    dims = (4, 4, 4, 8)
+    F, U = fields(dims)
+    nrhs = 3
+    eta = np.stack([ti.z4(dims, seed=950 + r) for r in range(nrhs)])
+    eta[1, 2, 1, 3, 0, 1, 2] = np.nan
+    for prec in (4, 2):
+        pe = F.pack(eta, prec)
+        s = F.zeros_full(prec, nrhs)
+        ws = tm.device_buffer(tm.tm_cg_workspace_bytes(F.L, 8, prec, tm.TM_CG_LP_TRUNCATED, nrhs))
+        prm = tm.make_cg_params(KAPPA, MU, 1e-2, 200, tm.TM_CG_LP_TRUNCATED)
+        rc, info = tm.tm_cg_multi(F.L, None, 8, F.gauge(prec, 12), prec, 12, s, pe, prm, nrhs, ws)
+        assert rc == tm.TM_ERR_BREAKDOWN
+        assert [i.status for i in info] == [tm.TM_OK, tm.TM_ERR_BREAKDOWN, tm.TM_OK]
+        got = F.unpack(s, prec, nrhs=nrhs)
+        for r in (0, 2):
+            s_ref, _ = oracle.cg_solve(U, eta[r], KAPPA, MU, 1e-2, 200)
+            assert rel(got[r], s_ref) < 3e-2

@@ -118,3 +118,45 @@ def test_64x128_dslash_sampled_sites():
                 # per-site bound as well: no single sampled site may be off by more than 20x the field tolerance
                 worst = np.abs(got - ref).reshape(sites.size, -1).max(axis=1).max() / np.abs(ref).max()
                 assert worst < 20 * TOL[prec], (prec, recon, parity, worst)
+
+
+@pytest.mark.parametrize("prec", [4, 2])
+def test_32x64_insertions_full_size(prec):
+    """NEXT-2 / NEXT-3 kernels at the bench size (32^3x64, the launch shapes bench.py times): the covariant derivative on the
+    whole field, momentum-projected loops (123 momenta, p^2 <= 9) at sampled momenta against the plain phase sums, the zero
+    momentum against the time-slice loop kernel, the single-slice contraction, and (BH)^4 on the whole field."""
+    dims = (32, 32, 32, 64)
+    X, Y, Z, T = dims
+    U = ti.gauge(dims)
+    F = Fields(dims, U, True)
+    a, b = ti.z4(dims, seed=1201), ti.gauss_spinor(dims, 1202)
+    pa, pb_ = F.pack(a, prec), F.pack(b, prec)
+    # covariant derivative, mu = t (antiperiodic boundary) and mu = x (checkerboard shifts)
+    d = F.zeros_full(prec)
+    for mu in (3, 0):
+        tm.tm_covdev(F.L, F.gauge(prec, 12), prec, 12, d, pb_, mu, 1)
+        assert rel(F.unpack(d, prec), oracle.covdev(U, b, mu)) < TOL[prec]
+    # momentum-projected loops
+    mom = oracle.momenta_p2_max(9)
+    K = len(mom)
+    out = torch.zeros((1, 16, T, K, 2), dtype=torch.float64, device="cuda")
+    ws = tm.device_buffer(tm.tm_loop_momentum_workspace_bytes(F.L, 1, K, 3))
+    tm.tm_loop_momentum(F.L, pa, pb_, prec, 1, mom, out, ws)
+    got = out.cpu().numpy().view(np.complex128)[0, ..., 0]
+    sample = [0, 5, 61, 122]  # (0,0,0), a p^2 = 1, a mid-list and the last momentum
+    ref = oracle.loop_momentum(a, b, mom[sample])
+    for j, k in enumerate(sample):
+        assert rel(got[:, :, k], ref[:, :, j]) < TOL[prec], mom[k]
+    o2 = torch.zeros((1, 16, T, 2), dtype=torch.float64, device="cuda")
+    lws = tm.device_buffer(tm.tm_loop_workspace_bytes(F.L, 1))
+    tm.tm_loop_contract(F.L, pa, pb_, prec, 1, o2, lws)
+    k0 = [i for i, p in enumerate(mom) if tuple(p) == (0, 0, 0)][0]
+    assert rel(got[:, :, k0], o2.cpu().numpy().view(np.complex128)[0, ..., 0]) < 1e-6
+    # single-slice contraction
+    o3 = torch.zeros((1, 16, 2), dtype=torch.float64, device="cuda")
+    tm.tm_loop_contract_slice(F.L, pa, pb_, prec, 1, 37, o3, lws)
+    assert rel(o3.cpu().numpy().view(np.complex128)[0, ..., 0], oracle.loop_slice(a, b, 37)) < TOL[prec]
+    # hopping-parameter remainder
+    tmp = F.zeros_full(prec)
+    tm.tm_hpe_remainder(F.L, F.gauge(prec, 12), prec, 12, d, pb_, tmp, KAPPA, MU, 1)
+    assert rel(F.unpack(d, prec), oracle.hpe_remainder(U, b, KAPPA, MU)) < (4 if prec == 2 else 1) * TOL[prec]
