@@ -67,6 +67,7 @@ __device__ __forceinline__ void finish_scalar(const BlasCtx& c, int rhs, double 
         s.b2 = tot;
         s.rr = tot;
         if (!(tot > 0.0)) c.active[rhs] = 0; // zero source: x = 0 is the solution
+        if (!(tot == tot)) s.status = TM_ERR_BREAKDOWN; // NaN in the source
     } else if (FIN == FIN_PAP) {
         s.pAp = tot;
         s.alpha_iter = s.iter;

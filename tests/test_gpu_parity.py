@@ -85,7 +85,7 @@ def test_argument_errors():
             call()
         assert e.value.status == tm.TM_ERR_ARG
     with pytest.raises(tm.TmError) as e:
-        tm.tm_dslash(F.L, g, 4, 18, F.half(s, 4, 1)[16:], half, None, 0, 0, 0, KAPPA, MU)
+        tm.tm_dslash(F.L, g, 4, 18, F.half(s, 4, 1)[8:], half, None, 0, 0, 0, KAPPA, MU)  # not 16-byte aligned
     assert e.value.status == tm.TM_ERR_LAYOUT
 
 
