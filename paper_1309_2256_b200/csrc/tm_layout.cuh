@@ -29,6 +29,42 @@ __device__ __forceinline__ uint4 ldg128(const void* p) { return __ldg(reinterpre
 __device__ __forceinline__ uint2 ldg64(const void* p) { return __ldg(reinterpret_cast<const uint2*>(p)); }
 __device__ __forceinline__ uint32_t ldg32(const void* p) { return __ldg(reinterpret_cast<const uint32_t*>(p)); }
 
+// Link loads: every link is read exactly once per launch, so it is fetched with an L2 evict-first policy and without L1
+// allocation -- the neighbour spinors (each gathered by eight sites) keep the L2 (matters once the lattice outgrows it).
+#ifndef TM_LINK_STREAM
+#define TM_LINK_STREAM 1
+#endif
+__device__ __forceinline__ unsigned long long link_policy()
+{
+    unsigned long long pol;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+template <typename T>
+__device__ __forceinline__ T link_ldg(const T* p)
+{
+#if TM_LINK_STREAM
+    const unsigned long long pol = link_policy();
+    T v;
+    if constexpr (sizeof(T) == 16) {
+        uint4 q;
+        asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;" : "=r"(q.x), "=r"(q.y), "=r"(q.z), "=r"(q.w) : "l"(p), "l"(pol));
+        v = *reinterpret_cast<const T*>(&q);
+    } else if constexpr (sizeof(T) == 8) {
+        uint2 q;
+        asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.u32 {%0,%1}, [%2], %3;" : "=r"(q.x), "=r"(q.y) : "l"(p), "l"(pol));
+        v = *reinterpret_cast<const T*>(&q);
+    } else {
+        uint32_t q;
+        asm("ld.global.nc.L1::no_allocate.L2::cache_hint.u32 %0, [%1], %2;" : "=r"(q) : "l"(p), "l"(pol));
+        v = *reinterpret_cast<const T*>(&q);
+    }
+    return v;
+#else
+    return __ldg(p);
+#endif
+}
+
 __device__ __forceinline__ void unpack_h2(uint32_t w, float& a, float& b)
 {
     const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&w));
@@ -169,17 +205,17 @@ __device__ __forceinline__ void load_link(const void* block, int Vh, int cb, typ
             const double2* p = reinterpret_cast<const double2*>(block) + cb;
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                const double2 d = __ldg(p + (size_t)k * Vh);
+                const double2 d = link_ldg(p + (size_t)k * Vh);
                 q[2 * k] = d.x;
                 q[2 * k + 1] = d.y;
             }
         } else if constexpr (PREC == 4) {
             const float4* p = reinterpret_cast<const float4*>(block) + cb;
-            const float4 d0 = __ldg(p), d1 = __ldg(p + (size_t)Vh);
+            const float4 d0 = link_ldg(p), d1 = link_ldg(p + (size_t)Vh);
             q[0] = d0.x; q[1] = d0.y; q[2] = d0.z; q[3] = d0.w;
             q[4] = d1.x; q[5] = d1.y; q[6] = d1.z; q[7] = d1.w;
         } else {
-            const uint4 d = __ldg(reinterpret_cast<const uint4*>(block) + cb);
+            const uint4 d = link_ldg(reinterpret_cast<const uint4*>(block) + cb);
             unpack_h2(d.x, q[0], q[1]);
             unpack_h2(d.y, q[2], q[3]);
             unpack_h2(d.z, q[4], q[5]);
@@ -191,7 +227,7 @@ __device__ __forceinline__ void load_link(const void* block, int Vh, int cb, typ
         const double2* p = reinterpret_cast<const double2*>(block) + cb;
 #pragma unroll
         for (int k = 0; k < RECON / 2; ++k) {
-            const double2 d = __ldg(p + (size_t)k * Vh);
+            const double2 d = link_ldg(p + (size_t)k * Vh);
             u[2 * k] = d.x;
             u[2 * k + 1] = d.y;
         }
@@ -199,14 +235,14 @@ __device__ __forceinline__ void load_link(const void* block, int Vh, int cb, typ
         const float4* p = reinterpret_cast<const float4*>(block) + cb;
 #pragma unroll
         for (int k = 0; k < RECON / 4; ++k) {
-            const float4 d = __ldg(p + (size_t)k * Vh);
+            const float4 d = link_ldg(p + (size_t)k * Vh);
             u[4 * k] = d.x;
             u[4 * k + 1] = d.y;
             u[4 * k + 2] = d.z;
             u[4 * k + 3] = d.w;
         }
         if constexpr (RECON == 18) {
-            const float2 d = __ldg(reinterpret_cast<const float2*>(reinterpret_cast<const float4*>(block) + (size_t)4 * Vh) + cb);
+            const float2 d = link_ldg(reinterpret_cast<const float2*>(reinterpret_cast<const float4*>(block) + (size_t)4 * Vh) + cb);
             u[16] = d.x;
             u[17] = d.y;
         }
@@ -215,7 +251,7 @@ __device__ __forceinline__ void load_link(const void* block, int Vh, int cb, typ
         constexpr int NC = RECON / 8; // 2 or 1 full chunks
 #pragma unroll
         for (int k = 0; k < NC; ++k) {
-            const uint4 q = __ldg(p + (size_t)k * Vh);
+            const uint4 q = link_ldg(p + (size_t)k * Vh);
             unpack_h2(q.x, u[8 * k + 0], u[8 * k + 1]);
             unpack_h2(q.y, u[8 * k + 2], u[8 * k + 3]);
             unpack_h2(q.z, u[8 * k + 4], u[8 * k + 5]);
@@ -223,9 +259,9 @@ __device__ __forceinline__ void load_link(const void* block, int Vh, int cb, typ
         }
         const void* tail = reinterpret_cast<const uint4*>(block) + (size_t)NC * Vh;
         if constexpr (RECON == 18) {
-            unpack_h2(ldg32(reinterpret_cast<const uint32_t*>(tail) + cb), u[16], u[17]);
+            unpack_h2(link_ldg(reinterpret_cast<const uint32_t*>(tail) + cb), u[16], u[17]);
         } else {
-            const uint2 q = ldg64(reinterpret_cast<const uint2*>(tail) + cb);
+            const uint2 q = link_ldg(reinterpret_cast<const uint2*>(tail) + cb);
             unpack_h2(q.x, u[8], u[9]);
             unpack_h2(q.y, u[10], u[11]);
         }
