@@ -144,7 +144,7 @@ __device__ __forceinline__ void fused_axpy(const DslashKArgs& a, int rhs, int cb
 {
     typedef typename Prec<PREC>::real real;
     real y[24];
-    load_spinor<PREC>(a.axpy_y + (size_t)rhs * a.stride_y, a.g.Vh, cb, y);
+    load_spinor<PREC, true>(a.axpy_y + (size_t)rhs * a.stride_y, a.g.Vh, cb, y);
     const real c = (real)(*reinterpret_cast<const double*>(a.axpy_coef + (size_t)rhs * a.stride_coef));
 #pragma unroll
     for (int k = 0; k < 24; ++k) o[k] = fma(-c, o[k], y[k]);
@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(256) dslash_kernel(const DslashKArgs a)
         }
         if (a.x != nullptr) {
             real xv[24];
-            load_spinor<PREC>(a.x + (size_t)(r0 + r) * a.stride_x, Vh, cb, xv);
+            load_spinor<PREC, true>(a.x + (size_t)(r0 + r) * a.stride_x, Vh, cb, xv);
 #pragma unroll
             for (int k = 0; k < 12; ++k) {
                 const real s5 = (k < 6) ? real(1) : real(-1);

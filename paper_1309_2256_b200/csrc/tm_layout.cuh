@@ -80,14 +80,15 @@ __device__ __forceinline__ uint32_t pack_h2(float a, float b)
 // ------------------------------------------------------------------------------------------------
 // spinor load: v[24] in arithmetic precision
 // ------------------------------------------------------------------------------------------------
-template <int PREC>
+// STREAM: the operand is read exactly once per launch (the x of an XPAY epilogue, the y of a fused axpy): evict-first like the links
+template <int PREC, bool STREAM = false>
 __device__ __forceinline__ void load_spinor(const void* base, int Vh, int cb, typename Prec<PREC>::real* v)
 {
     if constexpr (PREC == 8) {
         const double2* p = reinterpret_cast<const double2*>(base) + cb;
 #pragma unroll
         for (int k = 0; k < 12; ++k) {
-            const double2 d = __ldg(p + (size_t)k * Vh);
+            const double2 d = STREAM ? link_ldg(p + (size_t)k * Vh) : __ldg(p + (size_t)k * Vh);
             v[2 * k] = d.x;
             v[2 * k + 1] = d.y;
         }
@@ -95,7 +96,7 @@ __device__ __forceinline__ void load_spinor(const void* base, int Vh, int cb, ty
         const float4* p = reinterpret_cast<const float4*>(base) + cb;
 #pragma unroll
         for (int k = 0; k < 6; ++k) {
-            const float4 d = __ldg(p + (size_t)k * Vh);
+            const float4 d = STREAM ? link_ldg(p + (size_t)k * Vh) : __ldg(p + (size_t)k * Vh);
             v[4 * k] = d.x;
             v[4 * k + 1] = d.y;
             v[4 * k + 2] = d.z;
@@ -105,8 +106,9 @@ __device__ __forceinline__ void load_spinor(const void* base, int Vh, int cb, ty
         const uint4* p = reinterpret_cast<const uint4*>(base) + cb;
         uint4 q[3];
 #pragma unroll
-        for (int k = 0; k < 3; ++k) q[k] = __ldg(p + (size_t)k * Vh);
-        const float nrm = __ldg(reinterpret_cast<const float*>(reinterpret_cast<const uint4*>(base) + (size_t)3 * Vh) + cb);
+        for (int k = 0; k < 3; ++k) q[k] = STREAM ? link_ldg(p + (size_t)k * Vh) : __ldg(p + (size_t)k * Vh);
+        const float* np_ = reinterpret_cast<const float*>(reinterpret_cast<const uint4*>(base) + (size_t)3 * Vh) + cb;
+        const float nrm = STREAM ? link_ldg(np_) : __ldg(np_);
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             unpack_h2(q[k].x, v[8 * k + 0], v[8 * k + 1]);
