@@ -33,7 +33,7 @@ FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12          # 148 SMs x 128 FP32 
 
 
 # one `ncu --set full` capture of the dominant kernel (profiles/r01_ncu_dslash_fp16_recon12_12rhs.md), bytes per launch
-NCU_DRAM_BYTES_PER_LAUNCH = 2.6145e9
+NCU_DRAM_BYTES_PER_LAUNCH = 2.485e9
 
 
 def peaks():
@@ -377,6 +377,22 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
         del vin, vout, vtmp
     out["insertions_next2_next3"] = ins
     del a, b
+
+    # the truncated solve UNBATCHED (one source per call, single-rhs kernels): the batching gain of configs[3]
+    fb2 = tm.tm_spinor_bytes(L, 2, 1, 1)
+    e1, s1 = tm.device_buffer(fb2), tm.device_buffer(fb2)
+    tm.tm_spinor_pack(L, psi, 2, 1, e1)
+    ws1 = tm.device_buffer(tm.tm_cg_workspace_bytes(L, 8, 2, tm.TM_CG_LP_TRUNCATED, 1))
+    prm1 = tm.make_cg_params(kappa, mu, LP_TOL, 500, tm.TM_CG_LP_TRUNCATED, 0.1, 0, 1)
+    its = []
+    def lp1(i):
+        rc, info = tm.tm_cg(L, None, 8, gauges[(2, 12)], 2, 12, s1, e1, prm1, ws1)
+        its.append(info.iters)
+    lp1(0)
+    ms = time_events(torch, lp1, 5)
+    out["lp_unbatched_fp16_recon12"] = {"ms_per_solve": ms, "solves_per_s": 1e3 / ms, "iters": its[-1],
+                                        "batched_over_unbatched": out["value"] / (1e3 / ms)}
+    del e1, s1, ws1
 
     # mixed-precision CG to 1e-8 on one Z2xiZ2 source (configs[2]): fp64 reliable updates, fp32 and fp16 iterations
     cg = {}
