@@ -239,3 +239,17 @@ def hpe_series(U, eta, kappa, mu, ap=True):
 def hpe_local_traces(kappa, mu):
     """Per-site Tr[Gamma_n (B - BHB + (BH)^2 B - (BH)^3 B)]_xx, complex [16] (gauge independent)."""
     return _ins.hpe_local_traces(kappa, mu, np.array([gamma(m) for m in range(5)]), _Gammas())
+
+
+def Mpc_sym(U, psi, kappa, mu, parity=0, ap=True, dagger=False):
+    """Symmetric even-odd preconditioned operator, PAPER.md:376 Eq. (A3) lhs: M_sym = 1 - kappa^2 R^-1 Dslash R^-1 Dslash on
+    `parity` (full-lattice arrays, zero elsewhere); dagger: 1 - kappa^2 Dslash^dag R^-dag Dslash^dag R^-dag."""
+    a = 2 * kappa * mu
+    v = project(_c(psi), parity)
+    if not dagger:
+        w = twist(project(hop(U, v, ap=ap), 1 - parity), a, inverse=True)
+        w = twist(project(hop(U, w, ap=ap), parity), a, inverse=True)
+    else:
+        w = project(hop(U, twist(v, -a, inverse=True), ap=ap, dagger=True), 1 - parity)
+        w = project(hop(U, twist(w, -a, inverse=True), ap=ap, dagger=True), parity)
+    return v - kappa ** 2 * w

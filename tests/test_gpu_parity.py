@@ -275,3 +275,22 @@ def test_ragged_lattice_6x6x6x6(prec, recon):
     got = out.cpu().numpy().view(np.complex128)[..., 0]
     for r in (0, 7):
         assert rel(got[r], oracle.loop(x[r], psi[r])) < TOL[prec]
+
+
+@pytest.mark.parametrize("prec", [8, 4, 2])
+def test_symmetric_preconditioned_operator_from_the_general_epilogue(prec):
+    """PAPER.md:376 Eq. (A3): M_sym = 1 - kappa^2 R^-1 Dslash R^-1 Dslash is two launches of the same kernels (TWIST_INV, then the
+    general epilogue with p = 1, q = -kappa^2 R^-1); its normal operator is M_pc^dag M_pc / (1 + a^2) (pin P24), so CG needs
+    no separate symmetric mode."""
+    dims = (4, 6, 8, 10)
+    F, U = fields(dims)
+    v = ti.gauss_spinor(dims, 333)
+    pin = F.pack(v, prec)
+    t1, out = F.zeros_full(prec), F.zeros_full(prec)
+    a = 2 * KAPPA * MU
+    d = 1.0 / (1.0 + a * a)
+    g = F.gauge(prec, 12)
+    tm.tm_dslash(F.L, g, prec, 12, F.half(t1, prec, 1), F.half(pin, prec, 0), None, 1, 0, tm.TM_KIND_TWIST_INV, KAPPA, MU)
+    tm.tm_dslash_general(F.L, g, prec, 12, F.half(out, prec, 0), F.half(t1, prec, 1), F.half(pin, prec, 0), 0, 0,
+                         (1.0, 0.0, -KAPPA ** 2 * d, KAPPA ** 2 * a * d))
+    assert rel(F.unpack(out, prec), oracle.Mpc_sym(U, v, KAPPA, MU)) < TOL[prec]

@@ -223,3 +223,21 @@ def test_P23_hpe_local_traces_are_the_dense_ones(dense_hpe):
     # leading term alone: Tr[Gamma_n B] = 12/(1+a^2) for 1, -12 i a/(1+a^2) for g5 ; the (BH)^2 B term is O(kappa^2 a)
     assert abs(loc[0] - 12 / (1 + A * A)) < 1000 * KAPPA ** 2 * A ** 2
     assert abs(loc[15] + 12j * A / (1 + A * A)) < 200 * KAPPA ** 2 * A
+
+
+# ---- P24 symmetric preconditioning, PAPER.md:376 Eq. (A3) ----------------------------------------------------------
+def test_P24_symmetric_preconditioning_is_a_rescaling_of_the_normal_operator():
+    """M_sym = R^-1 M_pc and R^dag R = (1 + a^2) 1 for the degenerate twist R = 1 + i a g5, hence
+    M_sym^dag M_sym = M_pc^dag M_pc / (1 + a^2): CG on either normal system produces the same iterates, which is why the
+    library implements (A2) only (reading 7).  Checked with a large twist so that the factor is visible."""
+    dims = (4, 4, 6, 4)
+    U = ti.gauge(dims)
+    v = oracle.project(ti.gauss_spinor(dims, 5), 0)
+    phi = oracle.project(ti.gauss_spinor(dims, 6), 0)
+    for mu in (MU, 0.9):
+        a = 2 * KAPPA * mu
+        ms = oracle.Mpc_sym(U, v, KAPPA, mu)
+        assert rel(ms, oracle.twist(oracle.Mpc(U, v, KAPPA, mu), a, inverse=True)) < 1e-13      # M_sym = R^-1 M_pc
+        assert abs(vdot(phi, ms) - vdot(oracle.Mpc_sym(U, phi, KAPPA, mu, dagger=True), v)) < 1e-12 * abs(vdot(phi, phi))
+        lhs = oracle.Mpc_sym(U, ms, KAPPA, mu, dagger=True)
+        assert rel(lhs, oracle.MdagM(U, v, KAPPA, mu) / (1 + a * a)) < 1e-13
