@@ -95,6 +95,13 @@ int tm_spinor_pack_z4(const tm_lattice* L, const unsigned char* codes, int prec,
  * k = spin*3 + colour in bits 2k (re < 0) and 2k+1 (im < 0): 3 bytes per site instead of 12 on the host->device path. */
 int tm_spinor_pack_z4_bits(const tm_lattice* L, const unsigned char* codes3, int prec, int nrhs, void* packed_out, void* stream);
 
+/* Z2 x iZ2 noise sources made on the device ("creation of stochastic sources ... carried out on GPUs"): source r
+ * of the batch is the field the synthetic-input generator (tm_inputs, counter-based splitmix64 hash) gives for seed + r *
+ * seed_stride, bit-identical to its codes passed through tm_spinor_pack_z4; nothing crosses PCIe.  packed_out: DEVICE
+ * [nrhs][parity][...] at `prec`. */
+int tm_noise_z4(const tm_lattice* L, unsigned long long seed, unsigned long long seed_stride, int prec, int nrhs, void* packed_out,
+                void* stream);
+
 /* ---- a2+a3: hopping term with fused local epilogue ("fused CUDA kernels, such as R_oo^-1 Dslash_oe,
  *      (R_ee - kappa^2 Dslash_eo) (and their daggered analogues)") ----------------------------------------- */
 /* out (parity out_parity) = epilogue(Dslash_{out_parity <- other} in).  in/out/x: DEVICE one-parity packed spinors

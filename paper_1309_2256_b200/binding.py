@@ -24,7 +24,7 @@ ABI_SYMBOLS = [
     "tm_tsm_workspace_bytes", "tm_tsm_batch_host", "tm_launch_count", "tm_kernel_timing_enable",
     "tm_kernel_timing_read", "tm_covdev", "tm_contract_field", "tm_loop_momentum_workspace_bytes", "tm_loop_momentum",
     "tm_time_dilute", "tm_loop_contract_slice", "tm_hpe_remainder", "tm_hpe_local_traces", "tm_spinor_pack_z4_bits",
-    "tm_tsm_batch_host_bits",
+    "tm_tsm_batch_host_bits", "tm_noise_z4",
 ]
 
 
@@ -100,6 +100,7 @@ def load():
         "tm_hpe_remainder": (i, [vp, vp, i, i, vp, vp, vp, d, d, i, vp]),
         "tm_hpe_local_traces": (i, [d, d, P(d)]),
         "tm_spinor_pack_z4_bits": (i, [vp, vp, i, i, vp, vp]),
+        "tm_noise_z4": (i, [vp, ctypes.c_ulonglong, ctypes.c_ulonglong, i, i, vp, vp]),
         "tm_tsm_batch_host_bits": (i, [vp, vp, i, i, vp, P(tm_cg_params), i, P(tm_cg_info), vp, vp, sz, vp]),
     }
     for name, (res, args) in sig.items():
@@ -338,12 +339,16 @@ def tm_spinor_pack_z4_bits(L, codes3, prec, nrhs, packed_out, stream=None):
                   "tm_spinor_pack_z4_bits")
 
 
+def tm_noise_z4(L, seed, seed_stride, prec, nrhs, packed_out, stream=None):
+    return _check(load().tm_noise_z4(L.handle, int(seed), int(seed_stride), prec, nrhs, _ptr(packed_out), _stream(stream)), "tm_noise_z4")
+
+
 def tm_tsm_batch_host_bits(L, gauge_lp, prec_lp, recon, codes3_host, params, nrhs, loops_host, workspace, stream=None):
     info = (tm_cg_info * nrhs)()
     ws_bytes = workspace.numel() * workspace.element_size()
     rc = load().tm_tsm_batch_host_bits(L.handle, _ptr(gauge_lp), prec_lp, recon, _ptr(codes3_host), ctypes.byref(params), nrhs, info,
                                        _ptr(loops_host), _ptr(workspace), ws_bytes, _stream(stream))
-    _check(rc, "tm_tsm_batch_host_bits", allow=_SOFT)
+    _check(rc, "tm_tsm_batch_host_bits", "tm_noise_z4", allow=_SOFT)
     return rc, list(info)
 
 

@@ -122,6 +122,44 @@ __global__ void spinor_pack_kernel(Geo g, const double* __restrict__ src, double
     }
 }
 
+// ---- Z2 x iZ2 noise made on the device ("creation of stochastic sources ... carried out on GPUs") ------------
+// The library's own statement of the counter-based generator of the synthetic inputs (three chained splitmix64 rounds over
+// (seed, stream 2, site * 12 + component, draw 0); the two top bits are the signs of re and im): source r of a batch is the
+// field of seed + r * seed_stride, bit-identical to the host generator's codes fed through tm_spinor_pack_z4.
+__device__ __forceinline__ unsigned long long dev_splitmix64(unsigned long long z)
+{
+    z += 0x9E3779B97F4A7C15ULL;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    return z ^ (z >> 31);
+}
+
+template <int PREC>
+__global__ void noise_z4_kernel(Geo g, unsigned long long seed, unsigned long long seed_stride, char* packed, size_t parity_bytes)
+{
+    typedef typename Prec<PREC>::real real;
+    const int cb = blockIdx.x * blockDim.x + threadIdx.x;
+    const int parity = blockIdx.y, rhs = blockIdx.z;
+    if (cb >= g.Vh) return;
+    uint32_t row, xh, rem2, y, t, z;
+    g.dXh.divmod((uint32_t)cb, row, xh);
+    g.dY.divmod(row, rem2, y);
+    g.dZ.divmod(rem2, t, z);
+    const unsigned long long site = 2ull * (unsigned long long)cb + ((parity + y + z + t) & 1);
+    const unsigned long long s0 = dev_splitmix64((seed + (unsigned long long)rhs * seed_stride) ^ (2ull * 0xD6E8FEB86659FD93ULL));
+    const real r = (real)0.70710678118654752440;
+    real v[24];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+        unsigned long long h = dev_splitmix64(s0 ^ ((site * 12ull + (unsigned long long)k) * 0xA0761D6478BD642FULL));
+        h = dev_splitmix64(h); // draw 0: h ^ (0 * constant)
+        const unsigned code = (unsigned)(h >> 62);
+        v[2 * k] = (code & 1u) ? -r : r;
+        v[2 * k + 1] = (code & 2u) ? -r : r;
+    }
+    store_spinor<PREC>(packed + ((size_t)rhs * 2 + parity) * parity_bytes, g.Vh, cb, v);
+}
+
 template <int PREC>
 static int gauge_pack_t(const Geo& g, const double* U, int recon, void* out, int check, cudaStream_t st)
 {
@@ -223,4 +261,20 @@ extern "C" int tm_spinor_pack_z4_bits(const tm_lattice* L, const unsigned char* 
     if (!L || !codes3 || !out || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
     if (!aligned256(codes3) || !aligned256(out)) return TM_ERR_LAYOUT;
     return spinor_pack_any(L->g, L->V, prec, 3, nullptr, nullptr, codes3, out, nrhs, (cudaStream_t)stream);
+}
+
+extern "C" int tm_noise_z4(const tm_lattice* L, unsigned long long seed, unsigned long long seed_stride, int prec, int nrhs,
+                           void* packed_out, void* stream)
+{
+    if (!L || !packed_out || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
+    if (!aligned256(packed_out)) return TM_ERR_LAYOUT;
+    const Geo& g = L->g;
+    dim3 block(128), grid((g.Vh + 127) / 128, 2, nrhs);
+    const size_t pb = spinor_parity_bytes(g, prec);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (prec == 8) noise_z4_kernel<8><<<grid, block, 0, st>>>(g, seed, seed_stride, (char*)packed_out, pb);
+    else if (prec == 4) noise_z4_kernel<4><<<grid, block, 0, st>>>(g, seed, seed_stride, (char*)packed_out, pb);
+    else noise_z4_kernel<2><<<grid, block, 0, st>>>(g, seed, seed_stride, (char*)packed_out, pb);
+    TM_LAUNCH_CHECK("noise_z4_kernel");
+    return TM_OK;
 }

@@ -57,6 +57,20 @@ def test_z4_code_pack_matches_spinor_pack():
         assert rel(F.unpack(buf, prec, nrhs=2), ref) < (1e-15 if prec == 8 else 1e-7 if prec == 4 else 6e-4)
 
 
+@pytest.mark.parametrize("prec", [8, 4, 2])
+def test_device_noise_is_the_host_generator(prec):
+    """tm_noise_z4 (sources made on the GPU) == the host generator's codes through tm_spinor_pack_z4, bit for bit."""
+    dims = (4, 6, 8, 10)
+    F, _ = fields(dims)
+    nrhs, seed, stride = 3, 4242, 7
+    codes = np.stack([ti.z4_codes(dims, seed=seed + r * stride) for r in range(nrhs)])
+    a = tm.device_buffer(tm.tm_spinor_bytes(F.L, prec, 1, nrhs))
+    b = tm.device_buffer(tm.tm_spinor_bytes(F.L, prec, 1, nrhs))
+    tm.tm_spinor_pack_z4(F.L, to_dev(codes), prec, nrhs, a)
+    tm.tm_noise_z4(F.L, seed, stride, prec, nrhs, b)
+    assert torch.equal(a, b)
+
+
 def test_gauge_pack_rejects_non_su3_for_recon12():
     dims = (4, 4, 4, 4)
     U = ti.gauge(dims).copy()
