@@ -348,7 +348,7 @@ def tm_tsm_batch_host_bits(L, gauge_lp, prec_lp, recon, codes3_host, params, nrh
     ws_bytes = workspace.numel() * workspace.element_size()
     rc = load().tm_tsm_batch_host_bits(L.handle, _ptr(gauge_lp), prec_lp, recon, _ptr(codes3_host), ctypes.byref(params), nrhs, info,
                                        _ptr(loops_host), _ptr(workspace), ws_bytes, _stream(stream))
-    _check(rc, "tm_tsm_batch_host_bits", "tm_noise_z4", allow=_SOFT)
+    _check(rc, "tm_tsm_batch_host_bits", allow=_SOFT)
     return rc, list(info)
 
 
