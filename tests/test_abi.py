@@ -62,3 +62,48 @@ def test_no_cpu_fallback(tm):
     with pytest.raises(tm.TmError):
         tm.tm_dslash(L, a.ctypes.data // 256 * 256 + 256, 4, 18, a.ctypes.data // 256 * 256 + 512, a.ctypes.data // 256 * 256 + 1024,
                      None, 0, 0, 0, 0.1, 0.0, 1, stream=0)
+
+
+def test_every_wrapper_reaches_the_library(tm):
+    """Each Python wrapper marshals its arguments into the C call and turns the status into TmError: called with NULL for a
+    required pointer the LIBRARY must answer TM_ERR_ARG (no device needed); a TypeError here would be a wrapper bug."""
+    import numpy as np
+    import torch
+    L = tm.tm_lattice_create((4, 4, 4, 4))
+    buf = torch.zeros(1 << 12, dtype=torch.uint8)  # host memory: never dereferenced, the NULL argument is rejected first
+    prm = tm.make_cg_params(0.16, 0.005, 1e-2, 10, tm.TM_CG_LP_TRUNCATED)
+    mom = np.zeros((1, 3), dtype=np.int32)
+    calls = [
+        lambda: tm.tm_gauge_pack(L, None, 4, 18, buf, 1e-10, stream=0),
+        lambda: tm.tm_spinor_pack(L, None, 4, 1, buf, stream=0),
+        lambda: tm.tm_spinor_unpack(L, None, 4, 1, buf, stream=0),
+        lambda: tm.tm_spinor_pack_z4(L, None, 4, 1, buf, stream=0),
+        lambda: tm.tm_spinor_pack_z4_bits(L, None, 4, 1, buf, stream=0),
+        lambda: tm.tm_noise_z4(L, 1, 1, 4, 1, None, stream=0),
+        lambda: tm.tm_dslash(L, None, 4, 18, buf, buf, None, 0, 0, 0, 0.1, 0.0, 1, stream=0),
+        lambda: tm.tm_dslash_general(L, None, 4, 18, buf, buf, None, 0, 0, (0, 0, 1, 0), 1, stream=0),
+        lambda: tm.tm_MdagM(L, None, 4, 18, buf, buf, buf, 0, 0.1, 0.0, 1, stream=0),
+        lambda: tm.tm_M(L, None, 4, 18, buf, buf, 0.1, 0.0, 0, 1, stream=0),
+        lambda: tm.tm_cg_multi(L, None, 8, None, 4, 18, buf, buf, prm, 2, buf, stream=0),
+        lambda: tm.tm_cg(L, None, 8, None, 4, 18, buf, buf, prm, buf, stream=0),
+        lambda: tm.tm_loop_contract(L, None, buf, 4, 1, buf, buf, stream=0),
+        lambda: tm.tm_loop_contract_ex(L, None, buf, 4, 1, 1, 0, 2j, buf, buf, stream=0),
+        lambda: tm.tm_loop_contract_slice(L, None, buf, 4, 1, 0, buf, buf, stream=0),
+        lambda: tm.tm_loop_momentum(L, None, buf, 4, 1, mom, buf, buf, stream=0),
+        lambda: tm.tm_contract_field(L, None, buf, 4, 1, buf, stream=0),
+        lambda: tm.tm_covdev(L, None, 4, 18, buf, buf, 0, 1, stream=0),
+        lambda: tm.tm_time_dilute(L, None, 4, 1, [1, 0, 0, 0], buf, stream=0),
+        lambda: tm.tm_hpe_remainder(L, None, 4, 18, buf, buf, buf, 0.1, 0.0, 1, stream=0),
+        lambda: tm.tm_oneend_loops(L, None, 4, 18, None, tm.TM_ONEEND_TAU3, 0.1, 0.0, 1, buf, buf, stream=0),
+        lambda: tm.tm_tsm_combine(4, None, None, 1, None, 0, buf, stream=0),
+        lambda: tm.tm_tsm_batch_host(L, None, 2, 12, buf, prm, 2, buf, buf, stream=0),
+        lambda: tm.tm_tsm_batch_host_bits(L, None, 2, 12, buf, prm, 2, buf, buf, stream=0),
+    ]
+    for k, call in enumerate(calls):
+        with pytest.raises(tm.TmError) as e:
+            call()
+        assert e.value.status == tm.TM_ERR_ARG, (k, e.value.status)
+    assert tm.tm_hpe_local_traces(0.16, 0.005).shape == (16,)
+    assert tm.tm_loop_momentum_workspace_bytes(L, 1, 1, 0) > 0 and tm.tm_oneend_workspace_bytes(L, 4, 1) > 0
+    assert tm.tm_tsm_workspace_bytes(L, 2, 2) > 0 and tm.tm_loop_workspace_bytes(L, 1) > 0
+    assert isinstance(tm.tm_launch_count(), int)
