@@ -205,7 +205,7 @@ __device__ __forceinline__ void hop_dir(const DslashKArgs& a, int cb, int nb, ty
 }
 
 template <int PREC, int RECON, int NR>
-__global__ void __launch_bounds__(256) dslash_kernel(const DslashKArgs a)
+__global__ void __launch_bounds__(256, PREC == 8 && NR == 1 ? 2 : 1) dslash_kernel(const DslashKArgs a)
 {
     typedef typename Prec<PREC>::real real;
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
