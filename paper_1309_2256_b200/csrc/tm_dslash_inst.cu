@@ -40,7 +40,7 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     const int n = p.nrhs;
     kernel_timing_begin(st);
 #if TM_PREC == 8
-    static const int cfg64 = getenv("TM_DSLASH_F64_NR") ? atoi(getenv("TM_DSLASH_F64_NR")) : 2;
+    static const int cfg64 = getenv("TM_DSLASH_F64_NR") ? atoi(getenv("TM_DSLASH_F64_NR")) : 1; // measured: one rhs per thread (links shared through L1) beats two at 128 registers
     if (n % 2 == 0 && cfg64 == 2) launch_nr<TM_PREC, TM_RECON, 2>(a, n / 2, st);
     else launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
 #else
