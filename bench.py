@@ -434,6 +434,16 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
         del ws
     del etaN, sN, c1
     out["cg_mixed_1e-8"] = cg
+    # the paper's per-configuration TSM workload (N_HP = 8, N_LP = 200) from the rates measured above
+    hp = cg.get("defect_x12_fp64+fp16")
+    if hp:
+        n_hp, n_lp = 8, 200
+        out["tsm_per_configuration"] = {
+            "n_hp": n_hp, "n_lp": n_lp, "seconds": n_hp * hp["ms_per_solve"] * 1e-3 + (n_hp + n_lp) / out["value"],
+            "R_HP_over_LP": hp["ms_per_solve"] * 1e-3 * out["value"],
+            "note": "derived: N_HP solves to 1e-8 (batched defect correction) + (N_HP + N_LP) truncated solves with their loops, at the "
+                    "rates measured in this run on the synthetic eps = 0.5 field (9 / 62 iterations; a physical light-quark ensemble "
+                    "needs about 10x more).  Context: PAPER.md Table I R_HP/LP = 17-27 (light, strange), Table II 1471 GPU-node-seconds"}
     if world == 1:
         base, _ = cpu_oracle_sample()
         out["cpu_baseline"] = base
