@@ -51,6 +51,49 @@ def test_32x64_twelve_rhs_dslash_whole_field():
             assert rel(got[r], ref) < TOL[prec], (kind, dagger, r)
 
 
+def test_32x64_tsm_step_through_the_link_cache():
+    """configs[3], the step bench.py times: 12 Z2xiZ2 sources from their codes -> batched truncated CG (tol 1e-2, fp16 storage,
+    12-real links: the 12-rhs kernel fed from the per-solve link cache by cp.async.bulk) -> 16-Gamma loops, at 32^3x64.
+    Checked against the oracle's CG on one source, the oracle's full operator and loop on the solutions, and the unbatched solve."""
+    dims = (32, 32, 32, 64)
+    nrhs, prec, recon = 12, 2, 12
+    U = ti.gauge(dims)
+    F = Fields(dims, U, True)
+    codes = np.stack([ti.z4_codes(dims, seed=ti.NOISE_SEED + r) for r in range(nrhs)])
+    pe = tm.device_buffer(tm.tm_spinor_bytes(F.L, prec, 1, nrhs))
+    tm.tm_spinor_pack_z4(F.L, to_dev(codes), prec, nrhs, pe)
+    del codes
+    g = F.gauge(prec, recon)
+    F.drop_canonical()
+    s = F.zeros_full(prec, nrhs)
+    ws = tm.device_buffer(tm.tm_cg_workspace_bytes(F.L, 8, prec, tm.TM_CG_LP_TRUNCATED, nrhs))
+    prm = tm.make_cg_params(KAPPA, MU, 1e-2, 500, tm.TM_CG_LP_TRUNCATED, 0.1, 0, 1)  # bench.py's parameters
+    rc, info = tm.tm_cg_multi(F.L, None, 8, g, prec, recon, s, pe, prm, nrhs, ws)
+    assert rc == tm.TM_OK
+    T = dims[3]
+    loops = torch.zeros((nrhs, 16, T, 2), dtype=torch.float64, device="cuda")
+    lws = tm.device_buffer(tm.tm_loop_workspace_bytes(F.L, nrhs))
+    tm.tm_loop_contract(F.L, pe, s, prec, nrhs, loops, lws)
+    loops = loops.cpu().numpy().view(np.complex128)[..., 0]
+    fb = tm.tm_spinor_bytes(F.L, prec, 1, 1)
+    s_ref, iref = oracle.cg_solve(U, ti.z4(dims, seed=ti.NOISE_SEED), KAPPA, MU, 1e-2, 500)
+    for r in (0, 11):
+        eta = ti.z4(dims, seed=ti.NOISE_SEED + r)
+        s_r = F.unpack(s[r * fb:(r + 1) * fb], prec)
+        assert info[r].status == tm.TM_OK and info[r].iterated_resid <= 1e-2
+        assert abs(info[r].iters - iref["iters"]) <= 1                               # P15
+        assert rel(oracle.M(U, s_r, KAPPA, MU), eta) < 1.3 * iref["true_resid_full"]  # the truncated residual, by the oracle's operator
+        assert rel(loops[r], oracle.loop(eta, s_r)) < TOL[prec]
+        if r == 0:
+            assert rel(s_r, s_ref) < 2e-2   # same x0 = 0 and the same steps up to storage rounding (as test_cg_lp_truncated_batched)
+        # the unbatched solve (single-rhs kernels, no link cache) gives the same bits
+        s1 = F.zeros_full(prec, 1)
+        ws1 = tm.device_buffer(tm.tm_cg_workspace_bytes(F.L, 8, prec, tm.TM_CG_LP_TRUNCATED, 1))
+        rc1, info1 = tm.tm_cg_multi(F.L, None, 8, g, prec, recon, s1, pe[r * fb:(r + 1) * fb], prm, 1, ws1)
+        assert rc1 == tm.TM_OK and info1[0].iters == info[r].iters
+        assert torch.equal(s1, s[r * fb:(r + 1) * fb])
+
+
 @pytest.mark.parametrize("prec,recon", [(4, 18), (4, 12), (2, 18), (2, 12)])
 def test_32x64_single_rhs_dslash_whole_field(prec, recon):
     """configs[2]: the single-rhs kernels bench.py's dslash table times."""
