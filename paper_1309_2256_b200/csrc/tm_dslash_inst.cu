@@ -1,6 +1,5 @@
 // tm_dslash_inst.cu -- one translation unit per (TM_PREC, TM_RECON), compiled with -DTM_PREC=.. -DTM_RECON=..
 #include "tm_dslash_tile.cuh"
-#include <cstdlib>
 
 #ifndef TM_PREC
 #error "compile with -DTM_PREC={8,4,2} -DTM_RECON={18,12}"
@@ -40,45 +39,22 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     const int n = p.nrhs;
     kernel_timing_begin(st);
 #if TM_PREC == 8
-    static const int cfg64 = getenv("TM_DSLASH_F64_NR") ? atoi(getenv("TM_DSLASH_F64_NR")) : 1; // measured: one rhs per thread (links shared through L1) beats two at 128 registers
-    if (n % 2 == 0 && cfg64 == 2) launch_nr<TM_PREC, TM_RECON, 2>(a, n / 2, st);
-    else launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
+    // fp64: one thread per (site, rhs); threads of one site share the link lines in L1 (measured faster than two rhs per
+    // thread at 128 registers)
+    launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
 #else
-    // Launch shapes from the B200 sweep; the environment knobs exist for re-tuning:
-    //   TM_DSLASH_SINGLE: 0 = 128 registers + prefetch, 1 = 128 registers (default), 2 = 96 registers + prefetch, -1 = dslash_kernel
-    //   TM_DSLASH_MULTI : 0 = by nrhs (12 / 6 / 4 right-hand sides per CTA at 80 registers), 1 = 12 + prefetch, -1 = dslash_kernel
-    static const int cfg_multi = getenv("TM_DSLASH_MULTI") ? atoi(getenv("TM_DSLASH_MULTI")) : 0;
-    static const int cfg_single = getenv("TM_DSLASH_SINGLE") ? atoi(getenv("TM_DSLASH_SINGLE")) : 1;
+    // Launch shapes from the B200 sweeps ("Optimisation log"):
+    //   1 rhs      128 sites per CTA, links per thread, packed fma.rn.f32x2 arithmetic, 4 CTAs/SM (128 registers)
+    //   2..4 rhs   32 sites x 4 rhs, links of the tile built in shared memory, 6 CTAs/SM
+    //   5..6 rhs   32 sites x 6 rhs, 4 CTAs/SM
+    //   > 6 rhs    32 sites x 12 rhs, 2 CTAs/SM (80 registers); inside a solve the tile images come from the link cache
+    //              by cp.async.bulk, 4 tiles per CTA
     const bool dg = p.dagger != 0;
-    if (n == 1) {
-        switch (cfg_single) {
-        case 0: launch_tile<TM_PREC, TM_RECON, 128, 1, 4, 0, true>(a, dg, st); break;
-        case 1: launch_tile<TM_PREC, TM_RECON, 128, 1, 4, 0, false>(a, dg, st); break;
-        case 2: launch_tile<TM_PREC, TM_RECON, 128, 1, 5, 0, true>(a, dg, st); break;
-        default: launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
-        }
-    } else if (cfg_multi == 0) {
-        if (n <= 4) launch_tile<TM_PREC, TM_RECON, 32, 4, 6, 1, false>(a, dg, st);
-        else if (n <= 6) launch_tile<TM_PREC, TM_RECON, 32, 6, 4, 1, false>(a, dg, st);
-        else if (a.link_cache) {
-            static const int tpc = getenv("TM_DSLASH_TPC") ? atoi(getenv("TM_DSLASH_TPC")) : 4;
-            static const int lcv = getenv("TM_DSLASH_LC") ? atoi(getenv("TM_DSLASH_LC")) : 0;
-            if (lcv == 1) launch_tile_lc<TM_PREC, TM_RECON, 6, 5, 4>(a, dg, st);
-            else if (lcv == 2) launch_tile_lc<TM_PREC, TM_RECON, 4, 8, 4>(a, dg, st);
-            else if (lcv == 3) launch_tile_lc<TM_PREC, TM_RECON, 6, 4, 4>(a, dg, st);
-            else if (tpc == 2) launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 2>(a, dg, st);
-            else if (tpc == 8) launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 8>(a, dg, st);
-            else launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 4>(a, dg, st);
-        }
-        else launch_tile<TM_PREC, TM_RECON, 32, 12, 2, 1, false>(a, dg, st);
-    } else if (cfg_multi == 1) {
-        launch_tile<TM_PREC, TM_RECON, 32, 12, 2, 1, true>(a, dg, st);
-    } else {
-        if (n % 3 == 0) launch_nr<TM_PREC, TM_RECON, 3>(a, n / 3, st);
-        else if (n % 4 == 0) launch_nr<TM_PREC, TM_RECON, 4>(a, n / 4, st);
-        else if (n % 2 == 0) launch_nr<TM_PREC, TM_RECON, 2>(a, n / 2, st);
-        else launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
-    }
+    if (n == 1) launch_tile<TM_PREC, TM_RECON, 128, 1, 4, 0, false>(a, dg, st);
+    else if (n <= 4) launch_tile<TM_PREC, TM_RECON, 32, 4, 6, 1, false>(a, dg, st);
+    else if (n <= 6) launch_tile<TM_PREC, TM_RECON, 32, 6, 4, 1, false>(a, dg, st);
+    else if (a.link_cache) launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 4>(a, dg, st);
+    else launch_tile<TM_PREC, TM_RECON, 32, 12, 2, 1, false>(a, dg, st);
 #endif
     kernel_timing_end(st);
     TM_LAUNCH_CHECK("dslash_kernel");
