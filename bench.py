@@ -394,6 +394,28 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
                                         "batched_over_unbatched": out["value"] / (1e3 / ms)}
     del e1, s1, ws1
 
+    # the same batched TSM step with fp32 storage ("inversions ... in single or half precision")
+    T = DIMS[3]
+    codes4 = torch.from_numpy(np.stack([ti.z4_codes(DIMS, seed=ti.NOISE_SEED + r) for r in range(NRHS)])).cuda()
+    fb4 = tm.tm_spinor_bytes(L, 4, 1, NRHS)
+    eta4, sol4 = tm.device_buffer(fb4), tm.device_buffer(fb4)
+    ws4 = tm.device_buffer(tm.tm_cg_workspace_bytes(L, 8, 4, tm.TM_CG_LP_TRUNCATED, NRHS))
+    lws4 = tm.device_buffer(tm.tm_loop_workspace_bytes(L, NRHS))
+    loops4 = torch.zeros((NRHS, 16, T, 2), dtype=torch.float64, device="cuda")
+    it4 = []
+
+    def step_fp32(i):
+        tm.tm_spinor_pack_z4(L, codes4, 4, NRHS, eta4)
+        rc, info = tm.tm_cg_multi(L, None, 8, gauges[(4, 12)], 4, 12, sol4, eta4, prm1, NRHS, ws4)
+        assert rc == tm.TM_OK, rc
+        tm.tm_loop_contract(L, eta4, sol4, 4, NRHS, loops4, lws4)
+        it4.append(info[0].iters)
+    step_fp32(0)
+    ms4 = time_events(torch, step_fp32, 3)
+    out["lp_batched_fp32_recon12"] = {"ms_per_step": ms4, "solves_per_s": NRHS / (ms4 * 1e-3), "iters": it4[-1],
+                                      "fp32_over_fp16_time": ms4 / out["ms_per_step"]}
+    del codes4, eta4, sol4, ws4, lws4, loops4
+
     # mixed-precision CG to 1e-8 on one Z2xiZ2 source (configs[2]): fp64 reliable updates, fp32 and fp16 iterations
     cg = {}
     pb8 = tm.tm_spinor_bytes(L, 8, 1, 1)
