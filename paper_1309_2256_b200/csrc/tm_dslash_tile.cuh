@@ -9,7 +9,7 @@
 //     converted to fp32, rebuilt from 12 reals, daggered for the backward hops, multiplied by the antiperiodic
 //     sign and parked in shared memory; the 8 neighbour indices of every site go there too.  All RB right-hand
 //     sides of the tile reuse them ("reuses each gauge link load", BASELINE.json north_star).
-//   phase B: per direction: raw 16-byte chunks of the neighbour (prefetched one direction ahead) -> spin
+//   phase B: per direction: raw 16-byte chunks of the neighbour -> spin
 //     projection to a half spinor (12 reals) -> SU(3) multiply -> reconstruction into the accumulator.
 // fp16 storage: the projection adds the binary16 words directly in fp32 (FHADD: f32 = f16 + f32, exact
 // inputs), and the per-site norm multiplies the 12 projected-and-rotated reals inside the reconstruction FMAs
@@ -207,7 +207,7 @@ struct TileSmem {
 
 // phase B + epilogue for one (site cb, right-hand side rhs): 8 hops from the neighbours nb[8], fused epilogue, store.
 // SL != 0: links come from the tile image `sm` (lane tx), already daggered and signed; SL == 0: loaded per thread.
-template <int PREC, int RECON, int DAG, int SL, bool PF, typename SM>
+template <int PREC, int RECON, int DAG, int SL, typename SM>
 __device__ __forceinline__ void tile_site(const DslashKArgs& a, const SM& sm, int cb, int tx, int rhs, const int* nb, float sgp,
                                           float sgm)
 {
@@ -219,17 +219,10 @@ __device__ __forceinline__ void tile_site(const DslashKArgs& a, const SM& sm, in
 #pragma unroll
     for (int k = 0; k < 24; ++k) acc[k] = 0.f;
 
-    Raw<PREC> cur, nxt;
-    if constexpr (PF) load_raw<PREC>(in, Vh, nb[0], nxt);
-
+    Raw<PREC> cur;
 #pragma unroll
     for (int d = 0; d < 8; ++d) {
-        if constexpr (PF) {
-            cur = nxt;
-            if (d < 7) load_raw<PREC>(in, Vh, nb[d + 1 < 8 ? d + 1 : 7], nxt);
-        } else {
-            load_raw<PREC>(in, Vh, nb[d], cur);
-        }
+        load_raw<PREC>(in, Vh, nb[d], cur); // (a register prefetch of direction d + 1 was measured: no gain at 80 / 128 registers)
         float u[18];
         if constexpr (SL) {
 #pragma unroll
@@ -405,7 +398,7 @@ __device__ __forceinline__ void tile_reconstruct2(f32x2* AU, f32x2* AL, const f3
     }
 }
 
-template <int PREC, int RECON, int DAG, int SL, bool PF, typename SM>
+template <int PREC, int RECON, int DAG, int SL, typename SM>
 __device__ __forceinline__ void tile_site2(const DslashKArgs& a, const SM& sm, int cb, int tx, int rhs, const int* nb, float sgp,
                                            float sgm)
 {
@@ -414,16 +407,10 @@ __device__ __forceinline__ void tile_site2(const DslashKArgs& a, const SM& sm, i
     const char* in = a.in + (size_t)rhs * a.stride_in;
     f32x2 AU[6], AL[6];
 
-    Raw<PREC> cur, nxt;
-    if constexpr (PF) load_raw<PREC>(in, Vh, nb[0], nxt);
+    Raw<PREC> cur;
 #pragma unroll
     for (int d = 0; d < 8; ++d) {
-        if constexpr (PF) {
-            cur = nxt;
-            if (d < 7) load_raw<PREC>(in, Vh, nb[d + 1 < 8 ? d + 1 : 7], nxt);
-        } else {
-            load_raw<PREC>(in, Vh, nb[d], cur);
-        }
+        load_raw<PREC>(in, Vh, nb[d], cur);
         float u[18];
         if constexpr (SL) {
 #pragma unroll
@@ -511,14 +498,14 @@ __device__ __forceinline__ void tile_site2(const DslashKArgs& a, const SM& sm, i
 #ifndef TM_F2
 #define TM_F2 1
 #endif
-template <int PREC, int RECON, int DAG, int SL, bool PF, typename SM>
+template <int PREC, int RECON, int DAG, int SL, typename SM>
 __device__ __forceinline__ void tile_site_any(const DslashKArgs& a, const SM& sm, int cb, int tx, int rhs, const int* nb, float sgp,
                                               float sgm)
 {
     // measured on B200: the packed form is 8-10 % faster where every thread also loads, converts and
     // rebuilds its own links (nrhs = 1) and 5 % slower in the multi-rhs kernels, whose FMA and LSU pipes are already balanced
-    if constexpr (TM_F2 == 1 ? SL == 0 : TM_F2 == 2) tile_site2<PREC, RECON, DAG, SL, PF>(a, sm, cb, tx, rhs, nb, sgp, sgm);
-    else tile_site<PREC, RECON, DAG, SL, PF>(a, sm, cb, tx, rhs, nb, sgp, sgm);
+    if constexpr (TM_F2 == 1 ? SL == 0 : TM_F2 == 2) tile_site2<PREC, RECON, DAG, SL>(a, sm, cb, tx, rhs, nb, sgp, sgm);
+    else tile_site<PREC, RECON, DAG, SL>(a, sm, cb, tx, rhs, nb, sgp, sgm);
 }
 
 // phase A for one tile: neighbour indices (the antiperiodic sign of a temporal hop rides on the index as ~index) and the
@@ -580,7 +567,7 @@ __global__ void __launch_bounds__(256) link_cache_kernel(DslashKArgs a, char* ca
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 // SL: 0 = links loaded by each thread (nrhs = 1), 1 = tile links built into shared memory in the kernel
-template <int PREC, int RECON, int DAG, int S, int RB, int MINB, int SL, bool PF>
+template <int PREC, int RECON, int DAG, int S, int RB, int MINB, int SL>
 __global__ void __launch_bounds__(S* RB, MINB) dslash_tile_kernel(const DslashKArgs a)
 {
     __shared__ __align__(128) TileSmem<SL ? S : 1> sm;
@@ -612,7 +599,7 @@ __global__ void __launch_bounds__(S* RB, MINB) dslash_tile_kernel(const DslashKA
         tile_neighbours(a.g, a.parity, cb, nb, sgp, sgm);
     }
 
-    tile_site_any<PREC, RECON, DAG, SL, PF>(a, sm, cb, tx, rhs, nb, sgp, sgm);
+    tile_site_any<PREC, RECON, DAG, SL>(a, sm, cb, tx, rhs, nb, sgp, sgm);
 }
 
 // ---- multi-rhs kernel fed from the link cache ------------------------------------------------------------------
@@ -674,7 +661,7 @@ __global__ void __launch_bounds__(32 * RB, MINB) dslash_tile_lc_kernel(const Dsl
                 const int v = sm[b].nbr[d][tx];
                 nb[d] = v < 0 ? ~v : v;
             }
-            tile_site_any<PREC, RECON, DAG, 1, false>(a, sm[b], cb, tx, rhs, nb, 1.f, 1.f);
+            tile_site_any<PREC, RECON, DAG, 1>(a, sm[b], cb, tx, rhs, nb, 1.f, 1.f);
         }
         if (i + 1 < ntile) __syncthreads();
     }
@@ -690,14 +677,14 @@ static inline void launch_tile_lc(const DslashKArgs& a, bool dagger, cudaStream_
     else dslash_tile_lc_kernel<PREC, RECON, 0, RB, MINB, TPC><<<grid, block, 0, st>>>(a);
 }
 
-template <int PREC, int RECON, int S, int RB, int MINB, int SL, bool PF>
+template <int PREC, int RECON, int S, int RB, int MINB, int SL>
 static inline void launch_tile(const DslashKArgs& a, bool dagger, cudaStream_t st)
 {
     const int ny = (a.nrhs + RB - 1) / RB;
     const unsigned tiles = (unsigned)((a.g.Vh + S - 1) / S);
     dim3 block(S, RB), grid(tiles * ny);
-    if (dagger) dslash_tile_kernel<PREC, RECON, 1, S, RB, MINB, SL, PF><<<grid, block, 0, st>>>(a);
-    else dslash_tile_kernel<PREC, RECON, 0, S, RB, MINB, SL, PF><<<grid, block, 0, st>>>(a);
+    if (dagger) dslash_tile_kernel<PREC, RECON, 1, S, RB, MINB, SL><<<grid, block, 0, st>>>(a);
+    else dslash_tile_kernel<PREC, RECON, 0, S, RB, MINB, SL><<<grid, block, 0, st>>>(a);
 }
 
 template <int PREC, int RECON>
