@@ -81,23 +81,25 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def cpu_oracle_sample():
-    """The oracle as it stands on the host cores: ONE complete truncated solve (tol 1e-2) + one 16-Gamma loop contraction on a
-    16^3x32 lattice (1/16 of the 32^3x64 sites, same generators/kappa/mu), scaled by the site ratio to solves/s at 32^3x64."""
+def cpu_oracle_sample(large=False):
+    """The oracle as it stands on the host cores: ONE complete truncated solve (tol 1e-2) + one 16-Gamma loop contraction, on a
+    lattice with the workload's generators / kappa / mu, scaled by the site ratio to solves/s at 32^3x64.
+    large: the 32^3x64 lattice of the workload itself (one of the 12 sources of a step, nothing extrapolated; 26 s on the 16 host
+    cores of the GPU box); else 16^3x32 (1/16 of the sites, 1.5 s: the per-step sample of --impl reference)."""
     import oracle
     import tm_inputs as ti
-    dims = (16, 16, 16, 32)
+    dims = DIMS if large else (16, 16, 16, 32)
     U = ti.gauge(dims)
     eta = ti.z4(dims)
     t0 = time.time()
     s, info = oracle.cg_solve(U, eta, ti.KAPPA, ti.MU, LP_TOL, 500)
     oracle.loop(eta, s)
     dt = time.time() - t0
-    scale = (32 ** 3 * 64) / (16 ** 3 * 32)
+    scale = float(np.prod(DIMS)) / float(np.prod(dims))
     cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    return {"value": 1.0 / (dt * scale), "unit": "solves/s", "cores": cores, "kind": "oracle",
-            "sample": "one truncated CG solve (tol 1e-2, %d iterations) + one 16-Gamma loop on 16^3x32 (1/16 of the sites) in %.1f s, "
-                      "scaled x1/16 to 32^3x64" % (info["iters"], dt)}, dt
+    sample = "one truncated CG solve (tol 1e-2, %d iterations) + one 16-Gamma loop on %dx%dx%dx%d in %.1f s" % ((info["iters"],) + tuple(dims) + (dt,))
+    sample += ": 1 of the 12 sources of a step, nothing extrapolated" if scale == 1.0 else " (1/%d of the sites), scaled x1/%d to 32^3x64" % (round(scale), round(scale))
+    return {"value": 1.0 / (dt * scale), "unit": "solves/s", "cores": cores, "kind": "oracle", "sample": sample}, dt
 
 
 def run_reference(args, rank):
@@ -155,7 +157,7 @@ def run_b200(args, rank, world, local_rank):
     # ---- once per configuration: gauge field -> packed links (a0) ----
     U = torch.from_numpy(ti.gauge(DIMS).view(np.float64)).cuda()
     gauges = {}
-    for prec, recon in ((2, 12), (2, 18), (4, 12), (4, 18), (8, 12), (8, 18), (2, 8), (4, 8), (8, 8)):
+    for prec, recon in ((2, 12), (2, 18), (4, 12), (4, 18), (8, 12), (8, 18), (2, 8), (4, 8), (8, 8), (2, 112), (2, 118)):
         gauges[(prec, recon)] = tm.device_buffer(tm.tm_gauge_bytes(L, prec, recon))
         tm.tm_gauge_pack(L, U, prec, recon, gauges[(prec, recon)], 1e-10)
     del U
@@ -295,8 +297,10 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
         for b in bufs + xs:
             b.copy_(src[:pb])
         tmp = tm.device_buffer(2 * pb)
-        for recon in (18, 12, 8):  # 8 = the paper's fastest reconstruction on the GTX Titan (Table A.1); ALU-bound on B200
+        # 8 = the paper's fastest reconstruction on the GTX Titan (Table A.1), ALU-bound on B200; 118 / 112 = 16-bit fixed-point links
+        for recon in (18, 12, 8) + ((118, 112) if prec == 2 else ()):
             g = gauges[(prec, recon)]
+            reals = recon % 100
             # "wilson_plain" = the hop alone (Table A.1's Wilson column: no twist in the epilogue)
             for kind, name, fl in ((tm.TM_KIND_TWIST_INV, "twist_inv", FLOPS_TWIST_INV), (tm.TM_KIND_XPAY_TWIST, "xpay_twist", FLOPS_XPAY),
                                    (tm.TM_KIND_PLAIN, "wilson_plain", 1320)):
@@ -306,11 +310,11 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
                 for i in range(5):
                     run(i)
                 ms = min(time_events(torch, run, 40) for _ in range(3))
-                by = dslash_bytes(Vh, prec, recon, kind == tm.TM_KIND_XPAY_TWIST)
+                by = dslash_bytes(Vh, prec, reals, kind == tm.TM_KIND_XPAY_TWIST)
                 sp = 24 * prec + (4 if prec == 2 else 0)
-                naive = Vh * (8 * recon * prec + (9 + (1 if kind == tm.TM_KIND_XPAY_TWIST else 0)) * sp)
+                naive = Vh * (8 * reals * prec + (9 + (1 if kind == tm.TM_KIND_XPAY_TWIST else 0)) * sp)
                 gbs = by / ms / 1e6
-                table["%s_fp%d_recon%d" % (name, prec * 8, recon)] = {
+                table["%s_fp%d_recon%d%s" % (name, prec * 8, reals, "fix16" if recon >= 100 else "")] = {
                     "us": ms * 1e3, "GFLOPS": Vh * fl / ms / 1e6, "GBps_algorithmic": gbs, "GBps_naive_model": naive / ms / 1e6,
                     "bytes_per_site_minimal": by / Vh, "bytes_per_site_naive": naive / Vh,
                     "frac_of_measured_%.0f" % hbm_peak: gbs / hbm_peak, "frac_of_nominal_8000": gbs / 8000.0}
@@ -414,7 +418,26 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
     ms4 = time_events(torch, step_fp32, 3)
     out["lp_batched_fp32_recon12"] = {"ms_per_step": ms4, "solves_per_s": NRHS / (ms4 * 1e-3), "iters": it4[-1],
                                       "fp32_over_fp16_time": ms4 / out["ms_per_step"]}
-    del codes4, eta4, sol4, ws4, lws4, loops4
+    del eta4, sol4, ws4
+
+    # ... and with fp16 storage + 16-bit fixed-point links (TM_RECON_12_FIX16): the 12-rhs kernel reads the fp32 link cache, so the
+    # more accurate links cost nothing there
+    fbx = tm.tm_spinor_bytes(L, 2, 1, NRHS)
+    etax, solx = tm.device_buffer(fbx), tm.device_buffer(fbx)
+    wsx = tm.device_buffer(tm.tm_cg_workspace_bytes(L, 8, 2, tm.TM_CG_LP_TRUNCATED, NRHS))
+    itx = []
+
+    def step_fix16(i):
+        tm.tm_spinor_pack_z4(L, codes4, 2, NRHS, etax)
+        rc, info = tm.tm_cg_multi(L, None, 8, gauges[(2, 112)], 2, 112, solx, etax, prm1, NRHS, wsx)
+        assert rc == tm.TM_OK, rc
+        tm.tm_loop_contract(L, etax, solx, 2, NRHS, loops4, lws4)
+        itx.append(info[0].iters)
+    step_fix16(0)
+    msx = time_events(torch, step_fix16, 3)
+    out["lp_batched_fp16_recon12fix16"] = {"ms_per_step": msx, "solves_per_s": NRHS / (msx * 1e-3), "iters": itx[-1],
+                                           "fix16_over_binary16_time": msx / out["ms_per_step"]}
+    del codes4, etax, solx, wsx, lws4, loops4
 
     # mixed-precision CG to 1e-8 on one Z2xiZ2 source (configs[2]): fp64 reliable updates, fp32 and fp16 iterations
     cg = {}
@@ -467,7 +490,8 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
                     "rates measured in this run on the synthetic eps = 0.5 field (9 / 62 iterations; a physical light-quark ensemble "
                     "needs about 10x more).  Context: PAPER.md Table I R_HP/LP = 17-27 (light, strange), Table II 1471 GPU-node-seconds"}
     if world == 1:
-        base, _ = cpu_oracle_sample()
+        # ~26 s of oracle work on the GPU box; the --impl reference arm keeps the 1.5 s sample so that its K + W steps stay short
+        base, _ = cpu_oracle_sample(large=True)
         out["cpu_baseline"] = base
 
 

@@ -40,7 +40,12 @@ extern "C" {
 typedef struct tm_lattice tm_lattice; /* opaque host-side geometry descriptor */
 
 typedef enum { TM_PREC_F64 = 8, TM_PREC_F32 = 4, TM_PREC_F16 = 2 } tm_prec;   /* storage bytes per real */
-typedef enum { TM_RECON_18 = 18, TM_RECON_12 = 12, TM_RECON_8 = 8 } tm_recon; /* reals stored per link */
+/* reals stored per link.  The *_FIX16 codes (reals + 100) select 16-bit FIXED-POINT link words for
+ * TM_PREC_F16 fields (Fig. 4 names only "16-bit (half)" precision; the fixed-point word is SURVEY.md 8(f) NEXT-4's variant of it, reading 32): every stored real is
+ * the offset-binary word q + 32768, q = rint(32767 u) in [-32767, 32767], value q / 32767 (+-1 exact, absolute error <= 1.6e-5
+ * against up to 2.4e-4 for binary16 entries near 1); same bytes and chunk layout as the binary16 links.  With TM_PREC_F64 /
+ * TM_PREC_F32 the flag is ignored (the field is the plain 18 / 12-real one), so one `recon` serves a mixed-precision solve. */
+typedef enum { TM_RECON_18 = 18, TM_RECON_12 = 12, TM_RECON_8 = 8, TM_RECON_18_FIX16 = 118, TM_RECON_12_FIX16 = 112 } tm_recon;
 typedef enum { TM_KIND_PLAIN = 0, TM_KIND_TWIST_INV = 1, TM_KIND_XPAY_TWIST = 2 } tm_dslash_kind;
 typedef enum { TM_CG_HP_MIXED = 0, TM_CG_LP_TRUNCATED = 1, TM_CG_HP_DEFECT = 2 } tm_cg_mode;
 

@@ -51,13 +51,14 @@ void kernel_timing_end(cudaStream_t st)
 template <int PREC, int RECON>
 int launch_dslash_t(const Geo& g, const DslashParams& p, cudaStream_t st);
 #define TM_DECL(P, R) template <> int launch_dslash_t<P, R>(const Geo&, const DslashParams&, cudaStream_t);
-TM_DECL(8, 18) TM_DECL(8, 12) TM_DECL(4, 18) TM_DECL(4, 12) TM_DECL(2, 18) TM_DECL(2, 12)
+TM_DECL(8, 18) TM_DECL(8, 12) TM_DECL(8, 8) TM_DECL(4, 18) TM_DECL(4, 12) TM_DECL(4, 8) TM_DECL(2, 18) TM_DECL(2, 12) TM_DECL(2, 8)
+TM_DECL(2, 118) TM_DECL(2, 112)
 #undef TM_DECL
 
 template <int PREC, int RECON>
 int link_cache_build_t(const Geo& g, const void* gauge, void* cache, cudaStream_t st);
 #define TM_DECL_LC(P, R) template <> int link_cache_build_t<P, R>(const Geo&, const void*, void*, cudaStream_t);
-TM_DECL_LC(4, 18) TM_DECL_LC(4, 12) TM_DECL_LC(2, 18) TM_DECL_LC(2, 12)
+TM_DECL_LC(4, 18) TM_DECL_LC(4, 12) TM_DECL_LC(4, 8) TM_DECL_LC(2, 18) TM_DECL_LC(2, 12) TM_DECL_LC(2, 8) TM_DECL_LC(2, 118) TM_DECL_LC(2, 112)
 
 // sizeof(TileSmem<32>) = 8*32*4 + 8*4*32*16 + 8*32*8 bytes per 32-site tile, both parities
 size_t link_cache_bytes(const Geo& g, int prec)
@@ -68,15 +69,19 @@ size_t link_cache_bytes(const Geo& g, int prec)
 
 int link_cache_build(const Geo& g, int prec, int recon, const void* gauge, void* cache, cudaStream_t st)
 {
+    recon = link_recon(prec, recon);
     if (prec == 4) return recon == 18 ? link_cache_build_t<4, 18>(g, gauge, cache, st) : recon == 12 ? link_cache_build_t<4, 12>(g, gauge, cache, st) : link_cache_build_t<4, 8>(g, gauge, cache, st);
+    if (prec == 2 && recon >= 100) return recon == 118 ? link_cache_build_t<2, 118>(g, gauge, cache, st) : link_cache_build_t<2, 112>(g, gauge, cache, st);
     if (prec == 2) return recon == 18 ? link_cache_build_t<2, 18>(g, gauge, cache, st) : recon == 12 ? link_cache_build_t<2, 12>(g, gauge, cache, st) : link_cache_build_t<2, 8>(g, gauge, cache, st);
     return TM_ERR_ARG;
 }
 
 int launch_dslash(const Geo& g, int prec, int recon, const DslashParams& p, cudaStream_t st)
 {
+    recon = link_recon(prec, recon); // the fixed-point flag exists for 16-bit links only (tm.h)
     if (prec == 8) return recon == 18 ? launch_dslash_t<8, 18>(g, p, st) : recon == 12 ? launch_dslash_t<8, 12>(g, p, st) : launch_dslash_t<8, 8>(g, p, st);
     if (prec == 4) return recon == 18 ? launch_dslash_t<4, 18>(g, p, st) : recon == 12 ? launch_dslash_t<4, 12>(g, p, st) : launch_dslash_t<4, 8>(g, p, st);
+    if (recon >= 100) return recon == 118 ? launch_dslash_t<2, 118>(g, p, st) : launch_dslash_t<2, 112>(g, p, st);
     return recon == 18 ? launch_dslash_t<2, 18>(g, p, st) : recon == 12 ? launch_dslash_t<2, 12>(g, p, st) : launch_dslash_t<2, 8>(g, p, st);
 }
 

@@ -68,10 +68,12 @@ static inline size_t round256(size_t n) { return (n + 255) & ~size_t(255); }
 
 // bytes of one single-parity spinor / one (parity,mu) link block
 static inline size_t spinor_parity_bytes(const Geo& g, int prec) { return (size_t)g.Vh * 24 * prec + (prec == 2 ? (size_t)g.Vh * 4 : 0); }
-static inline size_t link_block_bytes(const Geo& g, int prec, int recon) { return (size_t)g.Vh * recon * prec; }
+static inline size_t link_block_bytes(const Geo& g, int prec, int recon) { return (size_t)g.Vh * (recon % 100) * prec; }
 
 static inline bool valid_prec(int p) { return p == 8 || p == 4 || p == 2; }
-static inline bool valid_recon(int r) { return r == 18 || r == 12 || r == 8; }
+static inline bool valid_recon(int r) { return r == 18 || r == 12 || r == 8 || r == 118 || r == 112; }
+// TM_RECON_*_FIX16 (reals + 100) means 16-bit fixed-point link words and exists for 16-bit storage only: plain recon otherwise
+static inline int link_recon(int prec, int recon) { return prec == 2 ? recon : recon % 100; }
 
 // ---- internal launchers (defined in their own .cu files) ----
 struct DslashParams {

@@ -77,6 +77,23 @@ __device__ __forceinline__ uint32_t pack_h2(float a, float b)
     return *reinterpret_cast<const uint32_t*>(&h);
 }
 
+// 16-bit fixed-point link words (TM_RECON_*_FIX16, tm.h): each half of w is the offset-binary word q + 32768 of a real q / 32767.
+// 0x4B000000 | word is the float 2^23 + word exactly, so one byte permute, one exact subtraction and one multiply convert
+// it on the FMA / ALU pipes (an I2F per real would queue on the quarter-rate conversion unit).
+__device__ __forceinline__ void unpack_q2(uint32_t w, float& a, float& b)
+{
+    const float fa = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7610));
+    const float fb = __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7632));
+    a = (fa - 8421376.0f) * (1.0f / 32767.0f);
+    b = (fb - 8421376.0f) * (1.0f / 32767.0f);
+}
+template <bool FX>
+__device__ __forceinline__ void unpack_w2(uint32_t w, float& a, float& b)
+{
+    if constexpr (FX) unpack_q2(w, a, b);
+    else unpack_h2(w, a, b);
+}
+
 // ------------------------------------------------------------------------------------------------
 // spinor load: v[24] in arithmetic precision
 // ------------------------------------------------------------------------------------------------
@@ -198,9 +215,12 @@ __device__ __forceinline__ void rebuild_from8(const real* q, real* u)
     rebuild_row2(u);
 }
 
-template <int PREC, int RECON>
+template <int PREC, int RECON_CODE>
 __device__ __forceinline__ void load_link(const void* block, int Vh, int cb, typename Prec<PREC>::real* u)
 {
+    constexpr int RECON = RECON_CODE % 100;                  // reals stored per link
+    constexpr bool FX = (RECON_CODE >= 100) && (PREC == 2);  // 16-bit words are fixed point instead of binary16
+    static_assert(RECON_CODE < 100 || RECON == 18 || RECON == 12, "fixed-point links: 18 or 12 reals");
     if constexpr (RECON == 8) {
         typename Prec<PREC>::real q[8];
         if constexpr (PREC == 8) {
@@ -254,18 +274,18 @@ __device__ __forceinline__ void load_link(const void* block, int Vh, int cb, typ
 #pragma unroll
         for (int k = 0; k < NC; ++k) {
             const uint4 q = link_ldg(p + (size_t)k * Vh);
-            unpack_h2(q.x, u[8 * k + 0], u[8 * k + 1]);
-            unpack_h2(q.y, u[8 * k + 2], u[8 * k + 3]);
-            unpack_h2(q.z, u[8 * k + 4], u[8 * k + 5]);
-            unpack_h2(q.w, u[8 * k + 6], u[8 * k + 7]);
+            unpack_w2<FX>(q.x, u[8 * k + 0], u[8 * k + 1]);
+            unpack_w2<FX>(q.y, u[8 * k + 2], u[8 * k + 3]);
+            unpack_w2<FX>(q.z, u[8 * k + 4], u[8 * k + 5]);
+            unpack_w2<FX>(q.w, u[8 * k + 6], u[8 * k + 7]);
         }
         const void* tail = reinterpret_cast<const uint4*>(block) + (size_t)NC * Vh;
         if constexpr (RECON == 18) {
-            unpack_h2(link_ldg(reinterpret_cast<const uint32_t*>(tail) + cb), u[16], u[17]);
+            unpack_w2<FX>(link_ldg(reinterpret_cast<const uint32_t*>(tail) + cb), u[16], u[17]);
         } else {
             const uint2 q = link_ldg(reinterpret_cast<const uint2*>(tail) + cb);
-            unpack_h2(q.x, u[8], u[9]);
-            unpack_h2(q.y, u[10], u[11]);
+            unpack_w2<FX>(q.x, u[8], u[9]);
+            unpack_w2<FX>(q.y, u[10], u[11]);
         }
     }
     if constexpr (RECON == 12) rebuild_row2(u);

@@ -6,7 +6,7 @@ namespace tmk {
 __device__ unsigned int g_su3_dev_bits; // max deviation from SU(3) seen by the last gauge pack (float bits)
 __device__ unsigned int g_r8_inv_bits;  // recon 8: max 1 / (|U01|^2 + |U02|^2) seen by the last gauge pack (float bits)
 
-template <int PREC>
+template <int PREC, bool FX = false> // FX: 16-bit fixed-point words (TM_RECON_*_FIX16, tm.h) instead of binary16
 __device__ __forceinline__ void store_reals(void* block, int Vh, int cb, const double* u, int n)
 {
     // generic element-wise store following the chunk layout of tm_layout.cuh (n reals per site)
@@ -25,13 +25,16 @@ __device__ __forceinline__ void store_reals(void* block, int Vh, int cb, const d
         }
         if (PREC == 8) *reinterpret_cast<double*>(dst) = u[r];
         else if (PREC == 4) *reinterpret_cast<float*>(dst) = (float)u[r];
+        else if (FX) *reinterpret_cast<unsigned short*>(dst) = (unsigned short)(32768 + (int)rint(fmin(1.0, fmax(-1.0, u[r])) * 32767.0));
         else *reinterpret_cast<__half*>(dst) = __float2half_rn((float)u[r]);
     }
 }
 
-template <int PREC, int RECON>
+template <int PREC, int RECON_CODE>
 __global__ void gauge_pack_kernel(Geo g, const double* __restrict__ U, char* out, size_t link_block, int check)
 {
+    constexpr int RECON = RECON_CODE % 100;
+    constexpr bool FX = RECON_CODE >= 100 && PREC == 2;
     const int cb = blockIdx.x * blockDim.x + threadIdx.x;
     const int pm = blockIdx.y; // parity*4 + mu
     if (cb >= g.Vh) return;
@@ -73,7 +76,7 @@ __global__ void gauge_pack_kernel(Geo g, const double* __restrict__ U, char* out
         store_reals<PREC>(out + (size_t)pm * link_block, g.Vh, cb, q, 8);
         return;
     }
-    store_reals<PREC>(out + (size_t)pm * link_block, g.Vh, cb, u, RECON);
+    store_reals<PREC, FX>(out + (size_t)pm * link_block, g.Vh, cb, u, RECON);
 }
 
 template <int PREC, int MODE> // MODE 0: pack from fp64 canonical, 1: unpack to fp64 canonical, 2: pack from Z2xiZ2 codes (one byte
@@ -166,6 +169,8 @@ static int gauge_pack_t(const Geo& g, const double* U, int recon, void* out, int
     dim3 block(128), grid((g.Vh + 127) / 128, 8);
     if (recon == 18) gauge_pack_kernel<PREC, 18><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 18), check);
     else if (recon == 8) gauge_pack_kernel<PREC, 8><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 8), check);
+    else if (recon == 118) gauge_pack_kernel<PREC, 118><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 18), check);
+    else if (recon == 112) gauge_pack_kernel<PREC, 112><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 12), check);
     else gauge_pack_kernel<PREC, 12><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 12), check);
     TM_LAUNCH_CHECK("gauge_pack_kernel");
     return TM_OK;
@@ -202,7 +207,8 @@ extern "C" int tm_gauge_pack(const tm_lattice* L, const double* U, int prec, int
     if (!L || !U || !out || !valid_prec(prec) || !valid_recon(recon)) return TM_ERR_ARG;
     if (!aligned256(U) || !aligned256(out)) return TM_ERR_LAYOUT;
     cudaStream_t st = (cudaStream_t)stream;
-    const int check = (recon != 18 && su3_tol > 0) ? 1 : 0;
+    recon = link_recon(prec, recon);
+    const int check = (recon % 100 != 18 && su3_tol > 0) ? 1 : 0;
     if (check) {
         const unsigned int zero = 0;
         TM_CUDA_CHECK(cudaMemcpyToSymbolAsync(g_su3_dev_bits, &zero, sizeof(zero), 0, cudaMemcpyHostToDevice, st));

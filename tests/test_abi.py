@@ -44,6 +44,8 @@ def test_lattice_and_sizes(tm):
     assert tm.tm_gauge_bytes(L, 4, 18) == 4 * V * 18 * 4 == 603979776
     assert tm.tm_gauge_bytes(L, 4, 12) == 4 * V * 12 * 4
     assert tm.tm_gauge_bytes(L, 2, 12) == 4 * V * 12 * 2
+    assert tm.tm_gauge_bytes(L, 2, tm.TM_RECON_12_FIX16) == 4 * V * 12 * 2 and tm.tm_gauge_bytes(L, 2, tm.TM_RECON_18_FIX16) == 4 * V * 18 * 2
+    assert tm.tm_gauge_bytes(L, 4, tm.TM_RECON_12_FIX16) == 4 * V * 12 * 4 and tm.tm_gauge_bytes(L, 2, 108) == 0  # flag ignored above 16 bits
     assert tm.tm_spinor_bytes(L, 8, 0, 1) == V // 2 * 24 * 8
     assert tm.tm_spinor_bytes(L, 2, 0, 1) == V // 2 * (24 * 2 + 4)
     assert tm.tm_spinor_bytes(L, 2, 1, 12) == 12 * V * (24 * 2 + 4)
