@@ -5,13 +5,6 @@
 #error "compile with -DTM_PREC={8,4,2} -DTM_RECON={18,12}"
 #endif
 
-#ifndef TM_S1
-#define TM_S1 128
-#endif
-#ifndef TM_MB1
-#define TM_MB1 4
-#endif
-
 namespace tmk {
 
 template <int PREC, int RECON>
@@ -57,7 +50,7 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     //   > 6 rhs    32 sites x 12 rhs, 2 CTAs/SM (80 registers); inside a solve the tile images come from the link cache
     //              by cp.async.bulk, 4 tiles per CTA
     const bool dg = p.dagger != 0;
-    if (n == 1) launch_tile<TM_PREC, TM_RECON, TM_S1, 1, TM_MB1, 0>(a, dg, st);
+    if (n == 1) launch_tile<TM_PREC, TM_RECON, 128, 1, 4, 0>(a, dg, st);
     else if (n <= 4) launch_tile<TM_PREC, TM_RECON, 32, 4, 6, 1>(a, dg, st);
     else if (n <= 6) launch_tile<TM_PREC, TM_RECON, 32, 6, 4, 1>(a, dg, st);
     else if (a.link_cache) launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 4>(a, dg, st);
