@@ -53,12 +53,18 @@ _lib = None
 
 
 def load():
-    """Load libtm_b200.so; fails loudly if it has not been built (python -m paper_1309_2256_b200.build)."""
+    """Load libtm_b200.so (built in-tree on first use if missing); fails loudly if it cannot be built."""
     global _lib
     if _lib is not None:
         return _lib
     if not os.path.exists(LIB_PATH):
-        raise ImportError("libtm_b200.so is missing: run `python -m paper_1309_2256_b200.build` (there is no CPU fallback)")
+        # a fresh checkout (built artefacts are not in the history): compile once with nvcc; still no CPU fallback
+        try:
+            from . import build as _build
+            _build.build()
+        except Exception as e:
+            raise ImportError("libtm_b200.so is missing and could not be built (python -m paper_1309_2256_b200.build): %s; "
+                              "there is no CPU fallback" % e) from e
     lib = ctypes.CDLL(LIB_PATH)
     vp, i, d, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
     P = ctypes.POINTER
