@@ -107,6 +107,8 @@ def run_reference(args, rank):
         return
     vals, dts = [], []
     base = None
+    for _ in range(args.warmup):  # untimed: library load, page faults of the first pass
+        cpu_oracle_sample()
     for _ in range(args.steps):
         base, dt = cpu_oracle_sample()
         vals.append(base["value"]); dts.append(dt)
