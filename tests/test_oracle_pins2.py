@@ -241,3 +241,33 @@ def test_P24_symmetric_preconditioning_is_a_rescaling_of_the_normal_operator():
         assert abs(vdot(phi, ms) - vdot(oracle.Mpc_sym(U, phi, KAPPA, mu, dagger=True), v)) < 1e-12 * abs(vdot(phi, phi))
         lhs = oracle.Mpc_sym(U, ms, KAPPA, mu, dagger=True)
         assert rel(lhs, oracle.MdagM(U, v, KAPPA, mu) / (1 + a * a)) < 1e-13
+
+
+def test_P25_temporal_gauge_is_a_gauge_transformation_of_the_oracle_operator():
+    """tm_inputs.temporal_gauge (a non-random, time-ordered transformation: g(x,t) = prod_{t'<t} U_t(x,t')) against the oracle:
+    U' stays in SU(3), U'_t = 1 on every slice but the last, the last slice carries the Polyakov loop (its trace equals that of the
+    ordered product of the original temporal links), M(U') g = g M(U) with the antiperiodic sign left on the fermions, and the
+    truncated CG takes the same number of iterations on both fields (the Krylov spaces are unitarily equivalent)."""
+    dims = (4, 4, 6, 8)
+    U = ti.gauge(dims)
+    Up, g = ti.temporal_gauge(U)
+    eye = np.eye(3)
+    assert np.abs(Up @ np.conj(np.swapaxes(Up, -1, -2)) - eye).max() < 1e-13
+    assert np.abs(np.linalg.det(Up) - 1).max() < 1e-13
+    assert not np.abs(Up[:-1, ..., 3, :, :] - eye).any()
+    P = np.broadcast_to(eye, U.shape[1:4] + (3, 3)).astype(np.complex128)
+    for t in range(dims[3]):
+        P = P @ U[t, ..., 3, :, :]
+    assert np.abs(np.trace(P, axis1=-2, axis2=-1) - np.trace(Up[-1, ..., 3, :, :], axis1=-2, axis2=-1)).max() < 1e-12
+    rot = lambda v: np.einsum("tzyxab,tzyxsb->tzyxsa", g, v)
+    psi = ti.gauss_spinor(dims, 41)
+    for dagger in (False, True):
+        lhs = oracle.M(Up, rot(psi), ti.KAPPA, ti.MU, ap=True, dagger=dagger)
+        rhs = rot(oracle.M(U, psi, ti.KAPPA, ti.MU, ap=True, dagger=dagger))
+        assert np.linalg.norm(lhs - rhs) / np.linalg.norm(rhs) < 1e-14
+    eta = ti.z4(dims, seed=5)
+    s0, i0 = oracle.cg_solve(U, eta, ti.KAPPA, ti.MU, 1e-6, 500)
+    s1, i1 = oracle.cg_solve(Up, rot(eta), ti.KAPPA, ti.MU, 1e-6, 500)
+    assert i0["iters"] == i1["iters"]
+    assert np.linalg.norm(s1 - rot(s0)) / np.linalg.norm(s0) < 1e-10
+    assert np.linalg.norm(oracle.loop(rot(eta), s1) - oracle.loop(eta, s0)) / np.linalg.norm(oracle.loop(eta, s0)) < 1e-10
