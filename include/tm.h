@@ -44,8 +44,14 @@ typedef enum { TM_PREC_F64 = 8, TM_PREC_F32 = 4, TM_PREC_F16 = 2 } tm_prec;   /*
  * TM_PREC_F16 fields (Fig. 4 names only "16-bit (half)" precision; the fixed-point word is SURVEY.md 8(f) NEXT-4's variant of it, reading 32): every stored real is
  * the offset-binary word q + 32768, q = rint(32767 u) in [-32767, 32767], value q / 32767 (+-1 exact, absolute error <= 1.6e-5
  * against up to 2.4e-4 for binary16 entries near 1); same bytes and chunk layout as the binary16 links.  With TM_PREC_F64 /
- * TM_PREC_F32 the flag is ignored (the field is the plain 18 / 12-real one), so one `recon` serves a mixed-precision solve. */
-typedef enum { TM_RECON_18 = 18, TM_RECON_12 = 12, TM_RECON_8 = 8, TM_RECON_18_FIX16 = 118, TM_RECON_12_FIX16 = 112 } tm_recon;
+ * TM_PREC_F32 the flag is ignored (the field is the plain 18 / 12-real one), so one `recon` serves a mixed-precision solve.
+ * The *_TG codes (reals + 200) DECLARE a field in temporal gauge: the temporal links of the slices t < T-1 are exactly the unit matrix (not in
+ * the paper; reading 33).  tm_gauge_pack verifies the declaration (TM_ERR_NOT_TGAUGE otherwise) and stores the field like the plain
+ * 18 / 12-real one -- unit links included, so a kernel that ignores the declaration is still correct.  The single-right-hand-side fp32 / fp16
+ * hopping-term kernels honour it: temporal hops that do not wrap around load no link and multiply by none (25 % fewer link bytes, 144
+ * fewer multiply-adds per site); every other kernel treats the code as the plain one. */
+typedef enum { TM_RECON_18 = 18, TM_RECON_12 = 12, TM_RECON_8 = 8, TM_RECON_18_FIX16 = 118, TM_RECON_12_FIX16 = 112,
+               TM_RECON_18_TG = 218, TM_RECON_12_TG = 212 } tm_recon;
 typedef enum { TM_KIND_PLAIN = 0, TM_KIND_TWIST_INV = 1, TM_KIND_XPAY_TWIST = 2 } tm_dslash_kind;
 typedef enum { TM_CG_HP_MIXED = 0, TM_CG_LP_TRUNCATED = 1, TM_CG_HP_DEFECT = 2 } tm_cg_mode;
 
@@ -57,7 +63,8 @@ typedef enum {
     TM_ERR_CUDA = -4,      /* CUDA runtime error (no device, launch failure); tm_last_cuda_error() has the text */
     TM_ERR_BREAKDOWN = -5, /* CG: <p,Ap> <= 0 or NaN */
     TM_ERR_MAXITER = -6,   /* CG: max_iter reached before tol (solution still returned) */
-    TM_ERR_RECON8 = -7     /* tm_gauge_pack with recon 8: a link has |U01|^2 + |U02|^2 < 1e-6, where the 8-real chart is singular */
+    TM_ERR_RECON8 = -7,    /* tm_gauge_pack with recon 8: a link has |U01|^2 + |U02|^2 < 1e-6, where the 8-real chart is singular */
+    TM_ERR_NOT_TGAUGE = -8 /* tm_gauge_pack with a *_TG code: a temporal link of a slice t < T-1 is not exactly the unit matrix */
 } tm_status;
 
 #define TM_MAX_NRHS 16

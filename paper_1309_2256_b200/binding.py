@@ -10,11 +10,13 @@ LIB_PATH = os.path.join(_HERE, "libtm_b200.so")
 
 TM_PREC_F64, TM_PREC_F32, TM_PREC_F16 = 8, 4, 2
 TM_RECON_18, TM_RECON_12, TM_RECON_8 = 18, 12, 8
+TM_RECON_18_TG, TM_RECON_12_TG = 218, 212  # field declared in temporal gauge (tm.h)
 TM_RECON_18_FIX16, TM_RECON_12_FIX16 = 118, 112  # 16-bit fixed-point link words for TM_PREC_F16 fields (tm.h)
 TM_KIND_PLAIN, TM_KIND_TWIST_INV, TM_KIND_XPAY_TWIST = 0, 1, 2
 TM_CG_HP_MIXED, TM_CG_LP_TRUNCATED, TM_CG_HP_DEFECT = 0, 1, 2
 TM_ONEEND_TAU3, TM_ONEEND_GENERAL = 0, 1
 TM_OK, TM_ERR_ARG, TM_ERR_LAYOUT, TM_ERR_NOT_SU3, TM_ERR_CUDA, TM_ERR_BREAKDOWN, TM_ERR_MAXITER, TM_ERR_RECON8 = 0, -1, -2, -3, -4, -5, -6, -7
+TM_ERR_NOT_TGAUGE = -8
 TM_MAX_NRHS = 16
 
 ABI_SYMBOLS = [

@@ -22,7 +22,7 @@ def _units():
         name = os.path.splitext(os.path.basename(src))[0]
         if name == "tm_dslash_inst":
             for prec in (8, 4, 2):
-                for recon in (18, 12, 8) + ((118, 112) if prec == 2 else ()):  # 1xx: 16-bit fixed-point links (tm.h)
+                for recon in (18, 12, 8) + ((118, 112) if prec == 2 else ()) + ((218, 212) if prec != 8 else ()):  # 1xx: fixed-point links, 2xx: temporal gauge (tm.h)
                     units.append((src, "%s_p%d_r%d.o" % (name, prec, recon), ["-DTM_PREC=%d" % prec, "-DTM_RECON=%d" % recon]))
         else:
             units.append((src, name + ".o", []))

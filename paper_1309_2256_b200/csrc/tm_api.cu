@@ -52,7 +52,7 @@ template <int PREC, int RECON>
 int launch_dslash_t(const Geo& g, const DslashParams& p, cudaStream_t st);
 #define TM_DECL(P, R) template <> int launch_dslash_t<P, R>(const Geo&, const DslashParams&, cudaStream_t);
 TM_DECL(8, 18) TM_DECL(8, 12) TM_DECL(8, 8) TM_DECL(4, 18) TM_DECL(4, 12) TM_DECL(4, 8) TM_DECL(2, 18) TM_DECL(2, 12) TM_DECL(2, 8)
-TM_DECL(2, 118) TM_DECL(2, 112)
+TM_DECL(2, 118) TM_DECL(2, 112) TM_DECL(4, 218) TM_DECL(4, 212) TM_DECL(2, 218) TM_DECL(2, 212)
 #undef TM_DECL
 
 template <int PREC, int RECON>
@@ -69,7 +69,7 @@ size_t link_cache_bytes(const Geo& g, int prec)
 
 int link_cache_build(const Geo& g, int prec, int recon, const void* gauge, void* cache, cudaStream_t st)
 {
-    recon = link_recon(prec, recon);
+    recon = stored_recon(prec, recon);
     if (prec == 4) return recon == 18 ? link_cache_build_t<4, 18>(g, gauge, cache, st) : recon == 12 ? link_cache_build_t<4, 12>(g, gauge, cache, st) : link_cache_build_t<4, 8>(g, gauge, cache, st);
     if (prec == 2 && recon >= 100) return recon == 118 ? link_cache_build_t<2, 118>(g, gauge, cache, st) : link_cache_build_t<2, 112>(g, gauge, cache, st);
     if (prec == 2) return recon == 18 ? link_cache_build_t<2, 18>(g, gauge, cache, st) : recon == 12 ? link_cache_build_t<2, 12>(g, gauge, cache, st) : link_cache_build_t<2, 8>(g, gauge, cache, st);
@@ -79,6 +79,13 @@ int link_cache_build(const Geo& g, int prec, int recon, const void* gauge, void*
 int launch_dslash(const Geo& g, int prec, int recon, const DslashParams& p, cudaStream_t st)
 {
     recon = link_recon(prec, recon); // the fixed-point flag exists for 16-bit links only (tm.h)
+    if (recon >= 200) { // temporal gauge declared: the single-rhs fp32 / fp16 kernels skip the unit links, the others read them
+        if (p.nrhs == 1) {
+            if (prec == 4) return recon == 218 ? launch_dslash_t<4, 218>(g, p, st) : launch_dslash_t<4, 212>(g, p, st);
+            return recon == 218 ? launch_dslash_t<2, 218>(g, p, st) : launch_dslash_t<2, 212>(g, p, st);
+        }
+        recon -= 200;
+    }
     if (prec == 8) return recon == 18 ? launch_dslash_t<8, 18>(g, p, st) : recon == 12 ? launch_dslash_t<8, 12>(g, p, st) : launch_dslash_t<8, 8>(g, p, st);
     if (prec == 4) return recon == 18 ? launch_dslash_t<4, 18>(g, p, st) : recon == 12 ? launch_dslash_t<4, 12>(g, p, st) : launch_dslash_t<4, 8>(g, p, st);
     if (recon >= 100) return recon == 118 ? launch_dslash_t<2, 118>(g, p, st) : launch_dslash_t<2, 112>(g, p, st);
@@ -98,6 +105,7 @@ extern "C" const char* tm_strerror(int s)
     case TM_ERR_ARG: return "invalid argument";
     case TM_ERR_LAYOUT: return "bad lattice dimensions, alignment or workspace size";
     case TM_ERR_NOT_SU3: return "gauge link is not SU(3) within su3_tol (required for 12- and 8-real storage)";
+    case TM_ERR_NOT_TGAUGE: return "a temporal link of a slice t < T-1 is not the unit matrix (field declared in temporal gauge)";
     case TM_ERR_RECON8: return "a gauge link lies where the 8-real parametrisation is singular (|U01|^2 + |U02|^2 < 1e-6)";
     case TM_ERR_CUDA: return "CUDA runtime error (see tm_last_cuda_error)";
     case TM_ERR_BREAKDOWN: return "CG breakdown (<p,Ap> <= 0 or NaN)";

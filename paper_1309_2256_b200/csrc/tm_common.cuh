@@ -71,9 +71,11 @@ static inline size_t spinor_parity_bytes(const Geo& g, int prec) { return (size_
 static inline size_t link_block_bytes(const Geo& g, int prec, int recon) { return (size_t)g.Vh * (recon % 100) * prec; }
 
 static inline bool valid_prec(int p) { return p == 8 || p == 4 || p == 2; }
-static inline bool valid_recon(int r) { return r == 18 || r == 12 || r == 8 || r == 118 || r == 112; }
-// TM_RECON_*_FIX16 (reals + 100) means 16-bit fixed-point link words and exists for 16-bit storage only: plain recon otherwise
-static inline int link_recon(int prec, int recon) { return prec == 2 ? recon : recon % 100; }
+static inline bool valid_recon(int r) { return r == 18 || r == 12 || r == 8 || r == 118 || r == 112 || r == 218 || r == 212; }
+// TM_RECON_*_FIX16 (reals + 100) means 16-bit fixed-point link words and exists for 16-bit storage only: plain recon otherwise.
+// TM_RECON_*_TG (reals + 200) declares temporal gauge; the field is stored like the plain one, fp64 kernels ignore the declaration.
+static inline int link_recon(int prec, int recon) { return recon >= 200 ? (prec == 8 ? recon - 200 : recon) : (prec == 2 ? recon : recon % 100); }
+static inline int stored_recon(int prec, int recon) { recon = link_recon(prec, recon); return recon >= 200 ? recon - 200 : recon; }
 
 // ---- internal launchers (defined in their own .cu files) ----
 struct DslashParams {

@@ -38,7 +38,12 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     for (int k = 0; k < 4; ++k) a.pq[k] = p.pq[k];
     const int n = p.nrhs;
     kernel_timing_begin(st);
-#if TM_PREC == 8
+#if TM_RECON >= 200
+    // temporal gauge declared (tm.h): the single-rhs kernel that loads no link for temporal hops inside the lattice; launch_dslash
+    // sends everything else to the plain instantiations
+    if (n != 1) return TM_ERR_ARG;
+    launch_tile<TM_PREC, TM_RECON, 128, 1, 4, 0>(a, p.dagger != 0, st);
+#elif TM_PREC == 8
     // fp64: one thread per (site, rhs); threads of one site share the link lines in L1 (measured faster than two rhs per
     // thread at 128 registers)
     launch_nr<TM_PREC, TM_RECON, 1>(a, n, st);
@@ -61,7 +66,7 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     return TM_OK;
 }
 
-#if TM_PREC != 8
+#if TM_PREC != 8 && TM_RECON < 200
 template <>
 int link_cache_build_t<TM_PREC, TM_RECON>(const Geo& g, const void* gauge, void* cache, cudaStream_t st)
 {

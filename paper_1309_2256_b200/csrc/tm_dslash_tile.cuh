@@ -427,7 +427,9 @@ __device__ __forceinline__ void tile_site2(const DslashKArgs& a, const SM& sm, i
         } else {
             const bool fwd = !(d & 1);
             const char* blk = a.gauge + (size_t)((fwd ? a.parity : 1 - a.parity) * 4 + (d >> 1)) * a.link_block;
-            load_link<PREC, RECON>(blk, Vh, fwd ? cb : nb[d], u);
+            // temporal gauge declared (RECON = reals + 200): a temporal hop that does not wrap around crosses a unit link
+            const bool unit_hop = RECON >= 200 && ((d == 6 && nb[6] > cb) || (d == 7 && nb[7] < cb));
+            if (!unit_hop) load_link<PREC, RECON>(blk, Vh, fwd ? cb : nb[d], u);
         }
         float h[12];
         float w = 1.f;
@@ -446,8 +448,14 @@ __device__ __forceinline__ void tile_site2(const DslashKArgs& a, const SM& sm, i
         if constexpr (SL) {
             su3_mul2<0>(u, H, G);
         } else {
-            if (d & 1) su3_mul2<1>(u, H, G);
-            else su3_mul2<0>(u, H, G);
+            if (RECON >= 200 && ((d == 6 && nb[6] > cb) || (d == 7 && nb[7] < cb))) {
+#pragma unroll
+                for (int k = 0; k < 6; ++k) G[k] = H[k];
+            } else if (d & 1) {
+                su3_mul2<1>(u, H, G);
+            } else {
+                su3_mul2<0>(u, H, G);
+            }
             if (d == 6) w *= sgp;
             if (d == 7) w *= sgm;
         }
@@ -504,6 +512,7 @@ __device__ __forceinline__ void tile_site_any(const DslashKArgs& a, const SM& sm
 {
     // measured on B200: the packed form is 8-10 % faster where every thread also loads, converts and
     // rebuilds its own links (nrhs = 1) and 5 % slower in the multi-rhs kernels, whose FMA and LSU pipes are already balanced
+    static_assert(RECON < 200 || (TM_F2 == 1 && SL == 0), "the temporal-gauge codes exist for the packed single-rhs form");
     if constexpr (TM_F2 == 1 ? SL == 0 : TM_F2 == 2) tile_site2<PREC, RECON, DAG, SL>(a, sm, cb, tx, rhs, nb, sgp, sgm);
     else tile_site<PREC, RECON, DAG, SL>(a, sm, cb, tx, rhs, nb, sgp, sgm);
 }

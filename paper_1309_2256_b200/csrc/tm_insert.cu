@@ -441,7 +441,7 @@ extern "C" int tm_covdev(const tm_lattice* L, const void* gauge, int prec, int r
     if (!aligned256(gauge) || !aligned256(out_full) || !aligned256(in_full)) return TM_ERR_LAYOUT;
     cudaStream_t st = (cudaStream_t)stream;
     const Geo& g = L->g;
-    recon = link_recon(prec, recon);
+    recon = stored_recon(prec, recon);
     if (recon >= 100) return recon == 118 ? covdev_launch<2, 118>(g, gauge, out_full, in_full, mu, nrhs, st) : covdev_launch<2, 112>(g, gauge, out_full, in_full, mu, nrhs, st);
 #define TM_COVDEV(P) (recon == 18 ? covdev_launch<P, 18>(g, gauge, out_full, in_full, mu, nrhs, st) : recon == 12 ? covdev_launch<P, 12>(g, gauge, out_full, in_full, mu, nrhs, st) : covdev_launch<P, 8>(g, gauge, out_full, in_full, mu, nrhs, st))
     if (prec == 8) return TM_COVDEV(8);

@@ -219,8 +219,8 @@ template <int PREC, int RECON_CODE>
 __device__ __forceinline__ void load_link(const void* block, int Vh, int cb, typename Prec<PREC>::real* u)
 {
     constexpr int RECON = RECON_CODE % 100;                  // reals stored per link
-    constexpr bool FX = (RECON_CODE >= 100) && (PREC == 2);  // 16-bit words are fixed point instead of binary16
-    static_assert(RECON_CODE < 100 || RECON == 18 || RECON == 12, "fixed-point links: 18 or 12 reals");
+    constexpr bool FX = (RECON_CODE / 100 == 1) && (PREC == 2); // 16-bit words are fixed point instead of binary16
+    static_assert(RECON_CODE < 100 || RECON == 18 || RECON == 12, "fixed-point / temporal-gauge codes: 18 or 12 reals");
     if constexpr (RECON == 8) {
         typename Prec<PREC>::real q[8];
         if constexpr (PREC == 8) {

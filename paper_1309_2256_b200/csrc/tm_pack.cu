@@ -5,6 +5,7 @@ namespace tmk {
 
 __device__ unsigned int g_su3_dev_bits; // max deviation from SU(3) seen by the last gauge pack (float bits)
 __device__ unsigned int g_r8_inv_bits;  // recon 8: max 1 / (|U01|^2 + |U02|^2) seen by the last gauge pack (float bits)
+__device__ unsigned int g_tg_bad;       // *_TG codes: number of temporal links of slices t < T-1 that are not exactly the unit matrix
 
 template <int PREC, bool FX = false> // FX: 16-bit fixed-point words (TM_RECON_*_FIX16, tm.h) instead of binary16
 __device__ __forceinline__ void store_reals(void* block, int Vh, int cb, const double* u, int n)
@@ -31,7 +32,7 @@ __device__ __forceinline__ void store_reals(void* block, int Vh, int cb, const d
 }
 
 template <int PREC, int RECON_CODE>
-__global__ void gauge_pack_kernel(Geo g, const double* __restrict__ U, char* out, size_t link_block, int check)
+__global__ void gauge_pack_kernel(Geo g, const double* __restrict__ U, char* out, size_t link_block, int check, int tgcheck)
 {
     constexpr int RECON = RECON_CODE % 100;
     constexpr bool FX = RECON_CODE >= 100 && PREC == 2;
@@ -48,6 +49,11 @@ __global__ void gauge_pack_kernel(Geo g, const double* __restrict__ U, char* out
     double u[18];
 #pragma unroll
     for (int k = 0; k < 18; ++k) u[k] = U[(site * 4 + mu) * 18 + k];
+    if (tgcheck && mu == 3 && (int)t < g.T - 1) { // declared temporal gauge (tm.h): exactly the unit matrix
+        bool one = true;
+        for (int k = 0; k < 18; ++k) one = one && (u[k] == ((k == 0 || k == 8 || k == 16) ? 1.0 : 0.0));
+        if (!one) atomicAdd(&g_tg_bad, 1u);
+    }
     if (check) {
         // deviation from SU(3): |U U^dag - 1|_max and |row2 - conj(row0 x row1)|_max
         double dev = 0;
@@ -164,14 +170,14 @@ __global__ void noise_z4_kernel(Geo g, unsigned long long seed, unsigned long lo
 }
 
 template <int PREC>
-static int gauge_pack_t(const Geo& g, const double* U, int recon, void* out, int check, cudaStream_t st)
+static int gauge_pack_t(const Geo& g, const double* U, int recon, void* out, int check, int tgcheck, cudaStream_t st)
 {
     dim3 block(128), grid((g.Vh + 127) / 128, 8);
-    if (recon == 18) gauge_pack_kernel<PREC, 18><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 18), check);
-    else if (recon == 8) gauge_pack_kernel<PREC, 8><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 8), check);
-    else if (recon == 118) gauge_pack_kernel<PREC, 118><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 18), check);
-    else if (recon == 112) gauge_pack_kernel<PREC, 112><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 12), check);
-    else gauge_pack_kernel<PREC, 12><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 12), check);
+    if (recon == 18) gauge_pack_kernel<PREC, 18><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 18), check, tgcheck);
+    else if (recon == 8) gauge_pack_kernel<PREC, 8><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 8), check, tgcheck);
+    else if (recon == 118) gauge_pack_kernel<PREC, 118><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 18), check, tgcheck);
+    else if (recon == 112) gauge_pack_kernel<PREC, 112><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 12), check, tgcheck);
+    else gauge_pack_kernel<PREC, 12><<<grid, block, 0, st>>>(g, U, (char*)out, link_block_bytes(g, PREC, 12), check, tgcheck);
     TM_LAUNCH_CHECK("gauge_pack_kernel");
     return TM_OK;
 }
@@ -207,8 +213,13 @@ extern "C" int tm_gauge_pack(const tm_lattice* L, const double* U, int prec, int
     if (!L || !U || !out || !valid_prec(prec) || !valid_recon(recon)) return TM_ERR_ARG;
     if (!aligned256(U) || !aligned256(out)) return TM_ERR_LAYOUT;
     cudaStream_t st = (cudaStream_t)stream;
-    recon = link_recon(prec, recon);
+    const int tgcheck = recon >= 200 ? 1 : 0; // declaration only: the field is stored like the plain 18 / 12-real one
+    recon = stored_recon(prec, recon);
     const int check = (recon % 100 != 18 && su3_tol > 0) ? 1 : 0;
+    if (tgcheck) {
+        const unsigned int zero = 0;
+        TM_CUDA_CHECK(cudaMemcpyToSymbolAsync(g_tg_bad, &zero, sizeof(zero), 0, cudaMemcpyHostToDevice, st));
+    }
     if (check) {
         const unsigned int zero = 0;
         TM_CUDA_CHECK(cudaMemcpyToSymbolAsync(g_su3_dev_bits, &zero, sizeof(zero), 0, cudaMemcpyHostToDevice, st));
@@ -218,10 +229,16 @@ extern "C" int tm_gauge_pack(const tm_lattice* L, const double* U, int prec, int
         TM_CUDA_CHECK(cudaMemcpyToSymbolAsync(g_r8_inv_bits, &zero, sizeof(zero), 0, cudaMemcpyHostToDevice, st));
     }
     int rc;
-    if (prec == 8) rc = gauge_pack_t<8>(L->g, U, recon, out, check, st);
-    else if (prec == 4) rc = gauge_pack_t<4>(L->g, U, recon, out, check, st);
-    else rc = gauge_pack_t<2>(L->g, U, recon, out, check, st);
+    if (prec == 8) rc = gauge_pack_t<8>(L->g, U, recon, out, check, tgcheck, st);
+    else if (prec == 4) rc = gauge_pack_t<4>(L->g, U, recon, out, check, tgcheck, st);
+    else rc = gauge_pack_t<2>(L->g, U, recon, out, check, tgcheck, st);
     if (rc != TM_OK) return rc;
+    if (tgcheck) { // this check always synchronises the stream
+        unsigned int bad = 0;
+        TM_CUDA_CHECK(cudaMemcpyFromSymbolAsync(&bad, g_tg_bad, sizeof(bad), 0, cudaMemcpyDeviceToHost, st));
+        TM_CUDA_CHECK(cudaStreamSynchronize(st));
+        if (bad != 0) return TM_ERR_NOT_TGAUGE;
+    }
     if (check) {
         unsigned int bits = 0;
         TM_CUDA_CHECK(cudaMemcpyFromSymbolAsync(&bits, g_su3_dev_bits, sizeof(bits), 0, cudaMemcpyDeviceToHost, st));
