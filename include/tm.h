@@ -95,6 +95,12 @@ size_t tm_spinor_bytes(const tm_lattice* L, int prec, int full, int nrhs);
 int tm_gauge_pack(const tm_lattice* L, const double* U_canonical, int prec, int recon, void* packed_out,
                   double su3_tol, void* stream);
 
+/* Temporal gauge (reading 33; not in the paper): g(x,t) = prod_{t' < t} U_t(x,t'), U'_mu(x) = g(x) U_mu(x) g(x+mu)^dag (periodic
+ * wrap; the antiperiodic sign belongs to the fermions).  U_canonical: DEVICE fp64 canonical field, transformed IN PLACE; the temporal links of
+ * the slices t < T-1 are written as exactly 1 (they are 1 up to rounding), slice T-1 carries the Polyakov loop.  g_out: DEVICE fp64
+ * [V][3][3][re,im], the transformation (eta' = g eta, s = g^dag s').  The result may be packed with TM_RECON_18_TG / TM_RECON_12_TG. */
+int tm_gauge_fix_temporal(const tm_lattice* L, double* U_canonical, double* g_out, void* stream);
+
 /* ---- a1: spinor pack / unpack (both parities, nrhs fields) ----------------------------------------------- */
 /* psi_canonical: DEVICE fp64 [nrhs][V][4][3][2]; packed: DEVICE [nrhs][parity][...] at `prec`.
  * fp16: per-site fp32 norm = max |re|,|im| over the site's 24 reals, components stored as x/norm (RN). */

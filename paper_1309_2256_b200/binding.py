@@ -27,7 +27,7 @@ ABI_SYMBOLS = [
     "tm_tsm_workspace_bytes", "tm_tsm_batch_host", "tm_launch_count", "tm_kernel_timing_enable",
     "tm_kernel_timing_read", "tm_covdev", "tm_contract_field", "tm_loop_momentum_workspace_bytes", "tm_loop_momentum",
     "tm_time_dilute", "tm_loop_contract_slice", "tm_hpe_remainder", "tm_hpe_local_traces", "tm_spinor_pack_z4_bits",
-    "tm_tsm_batch_host_bits", "tm_noise_z4",
+    "tm_tsm_batch_host_bits", "tm_noise_z4", "tm_gauge_fix_temporal",
 ]
 
 
@@ -110,6 +110,7 @@ def load():
         "tm_hpe_local_traces": (i, [d, d, P(d)]),
         "tm_spinor_pack_z4_bits": (i, [vp, vp, i, i, vp, vp]),
         "tm_noise_z4": (i, [vp, ctypes.c_ulonglong, ctypes.c_ulonglong, i, i, vp, vp]),
+        "tm_gauge_fix_temporal": (i, [vp, vp, vp, vp]),
         "tm_tsm_batch_host_bits": (i, [vp, vp, i, i, vp, P(tm_cg_params), i, P(tm_cg_info), vp, vp, sz, vp]),
     }
     for name, (res, args) in sig.items():
@@ -346,6 +347,10 @@ def tm_hpe_local_traces(kappa, mu):
 def tm_spinor_pack_z4_bits(L, codes3, prec, nrhs, packed_out, stream=None):
     return _check(load().tm_spinor_pack_z4_bits(L.handle, _ptr(codes3), prec, nrhs, _ptr(packed_out), _stream(stream)),
                   "tm_spinor_pack_z4_bits")
+
+
+def tm_gauge_fix_temporal(L, U_canonical, g_out, stream=None):
+    return _check(load().tm_gauge_fix_temporal(L.handle, _ptr(U_canonical), _ptr(g_out), _stream(stream)), "tm_gauge_fix_temporal")
 
 
 def tm_noise_z4(L, seed, seed_stride, prec, nrhs, packed_out, stream=None):

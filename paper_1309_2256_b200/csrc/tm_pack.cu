@@ -169,6 +169,62 @@ __global__ void noise_z4_kernel(Geo g, unsigned long long seed, unsigned long lo
     store_spinor<PREC>(packed + ((size_t)rhs * 2 + parity) * parity_bytes, g.Vh, cb, v);
 }
 
+// ---- temporal gauge (tm.h: tm_gauge_fix_temporal) -------------------------------------------------------------------------
+__device__ __forceinline__ void cmat_mul(const double* a, const double* b, double* c, bool bdag) // c = a b  or  a b^dag
+{
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) {
+            double re = 0.0, im = 0.0;
+            for (int k = 0; k < 3; ++k) {
+                const double ar = a[2 * (i * 3 + k)], ai = a[2 * (i * 3 + k) + 1];
+                const double br = bdag ? b[2 * (j * 3 + k)] : b[2 * (k * 3 + j)];
+                const double bi = bdag ? -b[2 * (j * 3 + k) + 1] : b[2 * (k * 3 + j) + 1];
+                re += ar * br - ai * bi;
+                im += ar * bi + ai * br;
+            }
+            c[2 * (i * 3 + j)] = re;
+            c[2 * (i * 3 + j) + 1] = im;
+        }
+}
+
+// one thread per spatial site: g(x, 0) = 1, g(x, t + 1) = g(x, t) U_t(x, t)
+__global__ void tgauge_g_kernel(Geo g, const double* __restrict__ U, double* __restrict__ G)
+{
+    const long long v3 = (long long)g.X * g.Y * g.Z;
+    const long long xs = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (xs >= v3) return;
+    double cur[18], nxt[18];
+    for (int k = 0; k < 18; ++k) cur[k] = (k == 0 || k == 8 || k == 16) ? 1.0 : 0.0;
+    for (int t = 0; t < g.T; ++t) {
+        const long long site = xs + v3 * t;
+        for (int k = 0; k < 18; ++k) G[site * 18 + k] = cur[k];
+        cmat_mul(cur, U + (site * 4 + 3) * 18, nxt, false);
+        for (int k = 0; k < 18; ++k) cur[k] = nxt[k];
+    }
+}
+
+// one thread per (site, mu): U'_mu(x) = g(x) U_mu(x) g(x + mu)^dag in place; temporal links inside the lattice are set to exactly 1
+__global__ void tgauge_apply_kernel(Geo g, double* U, const double* __restrict__ G, long long V)
+{
+    const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= 4 * V) return;
+    const long long site = id >> 2;
+    const int mu = (int)(id & 3);
+    const int ext[4] = {g.X, g.Y, g.Z, g.T};
+    const long long stride[4] = {1, g.X, (long long)g.X * g.Y, (long long)g.X * g.Y * g.Z};
+    const int c = (int)((site / stride[mu]) % ext[mu]);
+    const long long up = site + (c == ext[mu] - 1 ? -(long long)(ext[mu] - 1) : 1) * stride[mu];
+    double* u = U + id * 18;
+    if (mu == 3 && c < g.T - 1) {
+        for (int k = 0; k < 18; ++k) u[k] = (k == 0 || k == 8 || k == 16) ? 1.0 : 0.0;
+        return;
+    }
+    double a[18], b[18];
+    cmat_mul(G + site * 18, u, a, false);
+    cmat_mul(a, G + up * 18, b, true);
+    for (int k = 0; k < 18; ++k) u[k] = b[k];
+}
+
 template <int PREC>
 static int gauge_pack_t(const Geo& g, const double* U, int recon, void* out, int check, int tgcheck, cudaStream_t st)
 {
@@ -207,6 +263,19 @@ int spinor_pack_any(const Geo& g, long long V, int prec, int mode, const double*
 } // namespace tmk
 
 using namespace tmk;
+
+extern "C" int tm_gauge_fix_temporal(const tm_lattice* L, double* U, double* g_out, void* stream)
+{
+    if (!L || !U || !g_out) return TM_ERR_ARG;
+    if (!aligned256(U) || !aligned256(g_out)) return TM_ERR_LAYOUT;
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long v3 = (long long)L->g.X * L->g.Y * L->g.Z;
+    tgauge_g_kernel<<<(unsigned)((v3 + 127) / 128), 128, 0, st>>>(L->g, U, g_out);
+    TM_LAUNCH_CHECK("tgauge_g_kernel");
+    tgauge_apply_kernel<<<(unsigned)((4 * L->V + 127) / 128), 128, 0, st>>>(L->g, U, g_out, L->V);
+    TM_LAUNCH_CHECK("tgauge_apply_kernel");
+    return TM_OK;
+}
 
 extern "C" int tm_gauge_pack(const tm_lattice* L, const double* U, int prec, int recon, void* out, double su3_tol, void* stream)
 {

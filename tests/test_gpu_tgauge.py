@@ -86,3 +86,25 @@ def test_tg_multi_rhs_MdagM_and_solves(prec):
     assert rc == tm.TM_OK and info1[0].iters == info[3].iters and np.array_equal(s1, s[3])
     rc, infoh, sh = solve(F, eta[0], 8, prec, TG[12], tm.TM_CG_HP_MIXED, 1e-9, 3000)
     assert rc == tm.TM_OK and infoh[0].true_resid < 1e-9
+
+
+@pytest.mark.parametrize("dims", [(4, 6, 8, 10), (8, 8, 8, 16)])
+def test_gauge_fix_temporal_on_the_device(dims):
+    """tm_gauge_fix_temporal against the input-preparation routine pinned by P25 (tm_inputs.temporal_gauge): the transformed field and
+    the transformation to rounding, exact unit links where they belong, and the result is accepted under the temporal-gauge code."""
+    import torch
+    from tm_harness import to_dev
+    U0 = ti.gauge(dims)
+    U_ref, g_ref = ti.temporal_gauge(U0)
+    L = tm.tm_lattice_create(dims, True)
+    U_dev = to_dev(U0)
+    g_dev = torch.empty(L.V * 18, dtype=torch.float64, device="cuda")
+    tm.tm_gauge_fix_temporal(L, U_dev, g_dev)
+    torch.cuda.synchronize()
+    U_got = U_dev.cpu().numpy().view(np.complex128).reshape(U0.shape)
+    g_got = g_dev.cpu().numpy().view(np.complex128).reshape(g_ref.shape)
+    assert np.abs(g_got - g_ref).max() < 1e-13
+    assert np.abs(U_got - U_ref).max() < 1e-13
+    assert np.array_equal(U_got[:-1, ..., 3, :, :], U_ref[:-1, ..., 3, :, :])  # exactly 1
+    buf = tm.device_buffer(tm.tm_gauge_bytes(L, 4, TG[12]))
+    tm.tm_gauge_pack(L, U_dev, 4, TG[12], buf, 1e-10)  # raises on TM_ERR_NOT_TGAUGE / TM_ERR_NOT_SU3
