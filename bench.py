@@ -32,8 +32,20 @@ FLOPS_HOP, FLOPS_TWIST_INV, FLOPS_XPAY = 1320, 1392, 1416  # per output site (DE
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12          # 148 SMs x 128 FP32 lanes x 2 (FMA) x max SM clock
 
 
-# one `ncu --set full` capture of the dominant kernel (profiles/r01_ncu_dslash_fp16_recon12_12rhs.md), bytes per launch
-NCU_DRAM_BYTES_PER_LAUNCH = 2.485e9
+# DRAM bytes per launch of the dominant kernel: read from the tracked record of its `ncu --set full` capture, and only
+# trusted while the kernel the library launches still has the template signature that was profiled
+TRAFFIC_RECORD = os.path.join(ROOT, "profiles", "dominant_kernel_traffic.json")
+
+
+def ncu_traffic(signature):
+    """(bytes per launch | None, source string).  None when there is no record or it belongs to another kernel build."""
+    try:
+        rec = json.load(open(TRAFFIC_RECORD))
+    except Exception as e:
+        return None, "no usable %s (%s)" % (os.path.relpath(TRAFFIC_RECORD, ROOT), type(e).__name__)
+    if rec.get("signature") != signature:
+        return None, "stale: %s was captured for %r, the library launches %r" % (os.path.relpath(TRAFFIC_RECORD, ROOT), rec.get("signature"), signature)
+    return float(rec["dram_bytes_per_launch"]), "%s: %s" % (os.path.relpath(TRAFFIC_RECORD, ROOT), rec.get("source", ""))
 
 
 def peaks():
@@ -184,6 +196,7 @@ def run_b200(args, rank, world, local_rank):
     loops_host = torch.zeros((NRHS, 16, T, 2), dtype=torch.float64).pin_memory()
     prm = tm.make_cg_params(kappa, mu, LP_TOL, 500, tm.TM_CG_LP_TRUNCATED, 0.1, 0, 1)  # truncated mode: no residual recomputation
     iters_log = []
+    gather = shard.LoopGather(world * NRHS, NRHS, (16, T, 2), torch.float64, torch.device("cuda", local_rank)) if world > 1 else None
 
     def step(i):
         tm.tm_spinor_pack_z4(L, codes_dev[i % nb], prec, NRHS, eta)
@@ -191,7 +204,7 @@ def run_b200(args, rank, world, local_rank):
         assert rc == tm.TM_OK, rc
         tm.tm_loop_contract(L, eta, sol, prec, NRHS, loops, loop_ws)
         if world > 1:  # the path's only exchange: one gather of the [16][T] loops (16 KB per source), SURVEY.md 8(e)
-            shard.gather_loops(loops, world * NRHS, NRHS)
+            gather(loops)
         iters_log.append([x.iters for x in info])
 
     def step_e2e(i):
@@ -254,12 +267,14 @@ def run_b200(args, rank, world, local_rank):
     k_avg_ms = k_ms / max(1, k_n)
     ach_gbs = tot_bytes / (k_ms * 1e-3) / 1e9
     ach_tf = tot_flops / (k_ms * 1e-3) / 1e12
-    roofline = {"kernel": "dslash_tile_lc_kernel<fp16,recon12,12 rhs per CTA,4 tiles per CTA> (link cache + cp.async.bulk)", "bound": "alu", "achieved": ach_tf, "peak": FP32_PEAK_TFLOPS,
-                "unit": "TFLOP/s", "frac": ach_tf / FP32_PEAK_TFLOPS, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
-                "traffic_source": "profiles/r01_ncu_dslash_fp16_recon12_12rhs.md: dram__bytes_read.sum + dram__bytes_write.sum, mean of 4 launches (2 TWIST_INV, XPAY_TWIST + norm, XPAY_TWIST^dag + residual update; 12 active rhs, link cache); algorithmic mean 2.437e9",
+    sig = tm.tm_kernel_signature()
+    traffic, traffic_src = ncu_traffic(sig)
+    roofline = {"kernel": sig + " (fp16 storage, 12-real links, link cache + cp.async.bulk)", "bound": "alu", "achieved": ach_tf, "peak": FP32_PEAK_TFLOPS,
+                "unit": "TFLOP/s", "frac": ach_tf / FP32_PEAK_TFLOPS, "traffic": traffic, "traffic_source": traffic_src,
                 "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts and clocks)",
                 "avg_launch_ms": k_avg_ms, "launches_timed": int(k_n), "share_of_step": k_ms / (ms_step * args.steps),
-                "hbm_view": {"achieved_GBps": ach_gbs, "peak_GBps": hbm_peak, "frac": ach_gbs / hbm_peak, "peak_source": peak_src}}
+                # the same launches in the HBM view (flat scalars: nested objects do not survive the driver's parse)
+                "hbm_achieved_GBps": ach_gbs, "hbm_peak_GBps": hbm_peak, "hbm_frac": ach_gbs / hbm_peak, "hbm_peak_source": peak_src}
 
     out = {"metric": "LP solves/s", "value": value, "unit": "solves/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -276,6 +291,8 @@ def run_b200(args, rank, world, local_rank):
             del gauges, eta, sol, cg_ws, tsm_ws
             torch.cuda.empty_cache()
             sweep_other_configs(torch, tm, ti, hbm_peak, out)
+        if "dslash" in out:  # the single-rhs table goes last, so that the tail of the line holds it
+            out["dslash"] = out.pop("dslash")
         print(json.dumps(out))
     if world > 1:
         dist.barrier()
@@ -330,6 +347,15 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
         del bufs, xs, src, tmp
     out["dslash"] = table
     out["dslash_peak_source"] = peak_src
+    # BASELINE.json's first metric where the driver's parse keeps it: flat scalars inside `roofline` (TWIST_INV, 32^3x64, single rhs;
+    # algorithmic bytes / time as a fraction of the measured copy bandwidth; north_star's target is >= 0.70)
+    fk = "frac_of_measured_%.0f" % hbm_peak
+    for prec_, nm in ((4, "fp32"), (2, "fp16")):
+        for rc_ in (18, 12):
+            row = table["twist_inv_fp%d_recon%d" % (prec_ * 8, rc_)]
+            out["roofline"]["dslash_%s_r%d_frac" % (nm, rc_)] = row[fk]
+            out["roofline"]["dslash_%s_r%d_us" % (nm, rc_)] = row["us"]
+            out["roofline"]["dslash_%s_r%d_frac_of_8000" % (nm, rc_)] = row["frac_of_nominal_8000"]
 
     # the same single-rhs kernels on the temporal-gauge copy of the field, declared as such (TM_RECON_*_TG): temporal hops inside the
     # lattice load no link and multiply by none.  Bytes: 6 + 2/T links per site instead of 8; GFLOPS keep the 1320-flop convention.
@@ -623,6 +649,43 @@ def sweep_other_configs(torch, tm, ti, hbm_peak, out):
                              "table": big}
 
 
+def free_port():
+    import socket
+    sk = socket.socket()
+    sk.bind(("127.0.0.1", 0))
+    port = sk.getsockname()[1]
+    sk.close()
+    return port
+
+
+def run_dry(args, rank, world):
+    """--dry-run (CPU, gloo): the launcher and the N > 1 host logic without a GPU -- rendezvous, the source partition, the one
+    gather of the [16][T] loops, max-over-ranks of a time -- with stand-in loops that encode their source index."""
+    import torch
+    import torch.distributed as dist
+    from paper_1309_2256_b200 import shard
+    if world > 1:
+        dist.init_process_group("gloo")
+    T = DIMS[3]
+    n = world * NRHS
+    ids = shard.owned_sources(n, NRHS, rank, world)
+    local = torch.stack([torch.full((16, T, 2), float(r), dtype=torch.float64) for r in ids])
+    gather = shard.LoopGather(n, NRHS, (16, T, 2), torch.float64, torch.device("cpu"))
+    full = gather(local)
+    ok = bool(all(torch.all(full[r] == float(r)) for r in range(n)))
+    t = torch.tensor([float(rank + 1)], dtype=torch.float64)
+    ranks = [torch.zeros(1, dtype=torch.float64) for _ in range(world)]
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_gather(ranks, torch.tensor([float(rank)], dtype=torch.float64))
+    if rank == 0:
+        print(json.dumps({"dry_run": True, "n_gpus": world, "ranks_reported": [int(x.item()) for x in ranks], "gather_in_source_order": ok,
+                          "max_over_ranks": float(t.item()), "sources": n}))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -630,12 +693,27 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--sweeps", action="store_true", help="also time BASELINE.json configs[1] (16^3x32, CUDA graph) and [4] (64^3x128)")
+    ap.add_argument("--dry-run", action="store_true", help="CPU / gloo run of the launcher and the multi-rank host logic only (no GPU, no timing)")
     args = ap.parse_args()
+    if args.gpus < 1:
+        raise SystemExit("--gpus must be >= 1")
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl != "reference":
+        # started bare: launch one rank per GPU ourselves (the driver's torchrun line sets WORLD_SIZE and skips this)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus), "--master-addr", "127.0.0.1",
+               "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+        os.environ.setdefault("NCCL_DEBUG", "WARN")
+        sys.stdout.flush()
+        os.execv(sys.executable, cmd)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if world != args.gpus:
+        raise SystemExit("bench.py --gpus %d was started with WORLD_SIZE=%d: the rank count must equal --gpus" % (args.gpus, world))
+    if args.dry_run:
+        run_dry(args, rank, world)
         return
     if args.warmup < 3:
         args.warmup = 3

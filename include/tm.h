@@ -288,6 +288,10 @@ unsigned long long tm_launch_count(void);
  * synchronises and returns the accumulated milliseconds and launch count since the last reset. */
 int tm_kernel_timing_enable(int on);
 int tm_kernel_timing_read(double* ms_total, long long* launches, int reset);
+/* Name and template arguments (launch shape) of the kernel that dominates the batched truncated solve -- the 12-rhs fp16
+ * hopping term fed from the link cache -- as a static string.  bench.py quotes DRAM traffic from an ncu capture only while
+ * the capture was made with the same string (SURVEY.md 8(d) measurement). */
+const char* tm_kernel_signature(void);
 
 #ifdef __cplusplus
 }

@@ -27,7 +27,7 @@ ABI_SYMBOLS = [
     "tm_tsm_workspace_bytes", "tm_tsm_batch_host", "tm_launch_count", "tm_kernel_timing_enable",
     "tm_kernel_timing_read", "tm_covdev", "tm_contract_field", "tm_loop_momentum_workspace_bytes", "tm_loop_momentum",
     "tm_time_dilute", "tm_loop_contract_slice", "tm_hpe_remainder", "tm_hpe_local_traces", "tm_spinor_pack_z4_bits",
-    "tm_tsm_batch_host_bits", "tm_noise_z4", "tm_gauge_fix_temporal",
+    "tm_tsm_batch_host_bits", "tm_noise_z4", "tm_gauge_fix_temporal", "tm_kernel_signature",
 ]
 
 
@@ -100,6 +100,7 @@ def load():
         "tm_launch_count": (ctypes.c_ulonglong, []),
         "tm_kernel_timing_enable": (i, [i]),
         "tm_kernel_timing_read": (i, [P(d), P(ctypes.c_longlong), i]),
+        "tm_kernel_signature": (ctypes.c_char_p, []),
         "tm_covdev": (i, [vp, vp, i, i, vp, vp, i, i, vp]),
         "tm_contract_field": (i, [vp, vp, vp, i, i, vp, vp]),
         "tm_loop_momentum_workspace_bytes": (sz, [vp, i, i, i]),
@@ -379,6 +380,10 @@ def tm_kernel_timing_read(reset=True):
     n = ctypes.c_longlong()
     _check(load().tm_kernel_timing_read(ctypes.byref(ms), ctypes.byref(n), int(reset)), "tm_kernel_timing_read")
     return ms.value, n.value
+
+
+def tm_kernel_signature():
+    return load().tm_kernel_signature().decode()
 
 
 def device_buffer(nbytes, device="cuda"):

@@ -117,6 +117,9 @@ extern "C" const char* tm_strerror(int s)
 extern "C" const char* tm_last_cuda_error(void) { return g_cuda_err; }
 extern "C" unsigned long long tm_launch_count(void) { return g_launches.load(); }
 
+namespace tmk { const char* lc_kernel_signature(); }
+extern "C" const char* tm_kernel_signature(void) { return tmk::lc_kernel_signature(); }
+
 extern "C" int tm_kernel_timing_enable(int on)
 {
     std::lock_guard<std::mutex> lk(g_timing_mu);

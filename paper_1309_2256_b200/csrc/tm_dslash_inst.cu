@@ -1,8 +1,19 @@
 // tm_dslash_inst.cu -- one translation unit per (TM_PREC, TM_RECON), compiled with -DTM_PREC=.. -DTM_RECON=..
 #include "tm_dslash_tile.cuh"
+#include <cstdlib>
 
 #ifndef TM_PREC
 #error "compile with -DTM_PREC={8,4,2} -DTM_RECON={18,12}"
+#endif
+
+#ifndef TM_LC_RB
+#define TM_LC_RB 12
+#endif
+#ifndef TM_LC_MINB
+#define TM_LC_MINB 2
+#endif
+#ifndef TM_LC_TPC
+#define TM_LC_TPC 4
 #endif
 
 namespace tmk {
@@ -58,13 +69,37 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     if (n == 1) launch_tile<TM_PREC, TM_RECON, 128, 1, 4, 0>(a, dg, st);
     else if (n <= 4) launch_tile<TM_PREC, TM_RECON, 32, 4, 6, 1>(a, dg, st);
     else if (n <= 6) launch_tile<TM_PREC, TM_RECON, 32, 6, 4, 1>(a, dg, st);
-    else if (a.link_cache) launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 4>(a, dg, st);
+#ifdef TM_SWEEP
+    // probe builds only (_work/): the launch shape of the link-cache kernel is picked by the environment at run time
+    else if (a.link_cache) {
+        static const int cfg = getenv("TM_LC_CFG") ? atoi(getenv("TM_LC_CFG")) : 0;
+        switch (cfg) {
+#define TM_CASE(id, RB, MINB, TPC, RPT) case id: launch_tile_lc<TM_PREC, TM_RECON, RB, MINB, TPC, RPT>(a, dg, st); break;
+            TM_SWEEP_CASES
+#undef TM_CASE
+        default: launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 4, 1>(a, dg, st);
+        }
+    }
+#else
+    else if (a.link_cache) launch_tile_lc<TM_PREC, TM_RECON, TM_LC_RB, TM_LC_MINB, TM_LC_TPC>(a, dg, st);
+#endif
     else launch_tile<TM_PREC, TM_RECON, 32, 12, 2, 1>(a, dg, st);
 #endif
     kernel_timing_end(st);
     TM_LAUNCH_CHECK("dslash_kernel");
     return TM_OK;
 }
+
+#if TM_PREC == 2 && TM_RECON == 12
+// template signature of the kernel that dominates the TSM step (12 rhs, fp16 storage, 12-real links): bench.py ties the
+// DRAM traffic it quotes from an ncu capture to this string (tm_kernel_signature)
+#define TM_STR2(x) #x
+#define TM_STR(x) TM_STR2(x)
+const char* lc_kernel_signature()
+{
+    return "dslash_tile_lc_kernel<prec=2,recon=12,RB=" TM_STR(TM_LC_RB) ",MINB=" TM_STR(TM_LC_MINB) ",TPC=" TM_STR(TM_LC_TPC) ",RPT=" TM_STR(TM_LC_RPT) ">";
+}
+#endif
 
 #if TM_PREC != 8 && TM_RECON < 200
 template <>

@@ -205,6 +205,39 @@ struct TileSmem {
     float2 u2[8][S];
 };
 
+// fused epilogue of one (site, rhs): out = (p0 + i p1 g5) x + (q0 + i q1 g5) acc ; g5 = diag(1,1,-1,-1); optional residual
+// update, store, optional reduction partial
+template <int PREC>
+__device__ __forceinline__ void tile_epilogue(const DslashKArgs& a, int cb, int rhs, const float* acc)
+{
+    const int Vh = a.g.Vh;
+    const float p0 = (float)a.pq[0], p1 = (float)a.pq[1], q0 = (float)a.pq[2], q1 = (float)a.pq[3];
+    float o[24];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+        const float s5 = (k < 6) ? 1.f : -1.f;
+        const float dr = acc[2 * k], di = acc[2 * k + 1];
+        // explicit operation order: the packed variant (tile_site2) rounds identically, so a right-hand side gives the same
+        // bits whether it runs alone or in a batch
+        o[2 * k] = fmaf(-s5 * q1, di, q0 * dr);
+        o[2 * k + 1] = fmaf(s5 * q1, dr, q0 * di);
+    }
+    if (a.x != nullptr) {
+        float xv[24];
+        load_spinor<PREC, true>(a.x + (size_t)rhs * a.stride_x, Vh, cb, xv);
+#pragma unroll
+        for (int k = 0; k < 12; ++k) {
+            const float s5 = (k < 6) ? 1.f : -1.f;
+            o[2 * k] = fmaf(-s5 * p1, xv[2 * k + 1], fmaf(p0, xv[2 * k], o[2 * k]));
+            o[2 * k + 1] = fmaf(s5 * p1, xv[2 * k], fmaf(p0, xv[2 * k + 1], o[2 * k + 1]));
+        }
+    }
+    if (a.axpy_y != nullptr) fused_axpy<PREC>(a, rhs, cb, o);
+    store_spinor<PREC>(a.out + (size_t)rhs * a.stride_out, Vh, cb, o);
+    if (a.dot_partial != nullptr) warp_dot_store<PREC>(a, rhs, cb, o);
+}
+
+
 // phase B + epilogue for one (site cb, right-hand side rhs): 8 hops from the neighbours nb[8], fused epilogue, store.
 // SL != 0: links come from the tile image `sm` (lane tx), already daggered and signed; SL == 0: loaded per thread.
 template <int PREC, int RECON, int DAG, int SL, typename SM>
@@ -222,8 +255,23 @@ __device__ __forceinline__ void tile_site(const DslashKArgs& a, const SM& sm, in
     Raw<PREC> cur;
 #pragma unroll
     for (int d = 0; d < 8; ++d) {
+#ifdef TM_DEBUG_NOLDG // timing ablation (probe builds only, wrong results): no gather, the raw words come from registers
+        {
+            unsigned* w_ = reinterpret_cast<unsigned*>(&cur);
+#pragma unroll
+            for (int k = 0; k < (int)(sizeof(cur) / 4); ++k) w_[k] = 0x3c003800u + (unsigned)((nb[d] + k) & 0x3ff);
+            if constexpr (PREC == 2) cur.nrm = __int_as_float(0x3f800000 + (nb[d] & 0xffff));
+        }
+#else
         load_raw<PREC>(in, Vh, nb[d], cur); // (a register prefetch of direction d + 1 was measured: no gain at 80 / 128 registers)
+#endif
         float u[18];
+#ifdef TM_DEBUG_NOLDS // timing ablation (probe builds only, wrong results): no shared-memory link read
+        if constexpr (SL) {
+#pragma unroll
+            for (int k = 0; k < 18; ++k) u[k] = __int_as_float(0x3f000000 + nb[d] * 32 + k);
+        } else
+#endif
         if constexpr (SL) {
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
@@ -271,31 +319,66 @@ __device__ __forceinline__ void tile_site(const DslashKArgs& a, const SM& sm, in
         if (d == 7) tile_reconstruct<3, -E, true>(acc, g, w);
     }
 
-    // epilogue: out = (p0 + i p1 g5) x + (q0 + i q1 g5) acc ; g5 = diag(1,1,-1,-1)
-    const float p0 = (float)a.pq[0], p1 = (float)a.pq[1], q0 = (float)a.pq[2], q1 = (float)a.pq[3];
-    float o[24];
+    tile_epilogue<PREC>(a, cb, rhs, acc);
+}
+
+// ---- R right-hand sides per thread (multi-rhs kernels) -------------------------------------------------------
+// One thread owns a site and walks R right-hand sides inside the direction loop: the direction's 18 link reals are read
+// from the tile image ONCE and stay in registers for the R SU(3) products (4.5 LDS per R hops instead of per hop), the
+// neighbour index and its address arithmetic are shared, and the R gathers of a direction are in flight together.
+// Scalar FFMA with the operation order of tile_site, so every right-hand side gets the bits it gets alone.
+template <int PREC, int MUD, int E>
+__device__ __forceinline__ void tile_hop_acc(const Raw<PREC>& cur, const float* u, float* acc)
+{
+    float h[12], g[12];
+    float w = 1.f;
+    if constexpr (PREC == 2) w = cur.nrm;
+    tile_project<PREC, MUD, E>(cur, h);
+    su3_mul<0>(u, h, g);
+    tile_reconstruct<MUD, E, true>(acc, g, w);
+}
+
+template <int PREC, int RECON, int DAG, int R, typename SM>
+__device__ __forceinline__ void tile_site_r(const DslashKArgs& a, const SM& sm, int cb, int tx, int rhs0, const int* nb)
+{
+    constexpr int E = DAG ? -1 : 1;
+    const int Vh = a.g.Vh;
+    float acc[R][24];
 #pragma unroll
-    for (int k = 0; k < 12; ++k) {
-        const float s5 = (k < 6) ? 1.f : -1.f;
-        const float dr = acc[2 * k], di = acc[2 * k + 1];
-        // explicit operation order: the packed variant (tile_site2) rounds identically, so a right-hand side gives the same
-        // bits whether it runs alone or in a batch
-        o[2 * k] = fmaf(-s5 * q1, di, q0 * dr);
-        o[2 * k + 1] = fmaf(s5 * q1, dr, q0 * di);
-    }
-    if (a.x != nullptr) {
-        float xv[24];
-        load_spinor<PREC, true>(a.x + (size_t)rhs * a.stride_x, Vh, cb, xv);
+    for (int r = 0; r < R; ++r)
 #pragma unroll
-        for (int k = 0; k < 12; ++k) {
-            const float s5 = (k < 6) ? 1.f : -1.f;
-            o[2 * k] = fmaf(-s5 * p1, xv[2 * k + 1], fmaf(p0, xv[2 * k], o[2 * k]));
-            o[2 * k + 1] = fmaf(s5 * p1, xv[2 * k], fmaf(p0, xv[2 * k + 1], o[2 * k + 1]));
+        for (int k = 0; k < 24; ++k) acc[r][k] = 0.f;
+#pragma unroll
+    for (int d = 0; d < 8; ++d) {
+        Raw<PREC> cur[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) load_raw<PREC>(a.in + (size_t)(rhs0 + r) * a.stride_in, Vh, nb[d], cur[r]);
+        float u[18];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const float4 q = sm.u4[d][k][tx];
+            u[4 * k] = q.x;
+            u[4 * k + 1] = q.y;
+            u[4 * k + 2] = q.z;
+            u[4 * k + 3] = q.w;
+        }
+        const float2 q2 = sm.u2[d][tx];
+        u[16] = q2.x;
+        u[17] = q2.y;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (d == 0) tile_hop_acc<PREC, 0, E>(cur[r], u, acc[r]);
+            if (d == 1) tile_hop_acc<PREC, 0, -E>(cur[r], u, acc[r]);
+            if (d == 2) tile_hop_acc<PREC, 1, E>(cur[r], u, acc[r]);
+            if (d == 3) tile_hop_acc<PREC, 1, -E>(cur[r], u, acc[r]);
+            if (d == 4) tile_hop_acc<PREC, 2, E>(cur[r], u, acc[r]);
+            if (d == 5) tile_hop_acc<PREC, 2, -E>(cur[r], u, acc[r]);
+            if (d == 6) tile_hop_acc<PREC, 3, E>(cur[r], u, acc[r]);
+            if (d == 7) tile_hop_acc<PREC, 3, -E>(cur[r], u, acc[r]);
         }
     }
-    if (a.axpy_y != nullptr) fused_axpy<PREC>(a, rhs, cb, o);
-    store_spinor<PREC>(a.out + (size_t)rhs * a.stride_out, Vh, cb, o);
-    if (a.dot_partial != nullptr) warp_dot_store<PREC>(a, rhs, cb, o);
+#pragma unroll
+    for (int r = 0; r < R; ++r) tile_epilogue<PREC>(a, cb, rhs0 + r, acc[r]);
 }
 
 // ---- packed fp32x2 variant of phase B ----------------------------------------------------------------
@@ -606,6 +689,10 @@ __global__ void __launch_bounds__(S* RB, MINB) dslash_tile_kernel(const DslashKA
     if constexpr (!SL) {
         if (!act) return;
         tile_neighbours(a.g, a.parity, cb, nb, sgp, sgm);
+#ifdef TM_DEBUG_L1WIN // timing ablation (probe builds only, wrong results): every gather lands inside the CTA's own site range
+#pragma unroll
+        for (int d = 0; d < 8; ++d) nb[d] = min(cb0 + (nb[d] & (S - 1)), Vh - 1);
+#endif
     }
 
     tile_site_any<PREC, RECON, DAG, SL>(a, sm, cb, tx, rhs, nb, sgp, sgm);
@@ -631,9 +718,11 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
                  : "memory");
 }
 
-template <int PREC, int RECON, int DAG, int RB, int MINB, int TPC>
-__global__ void __launch_bounds__(32 * RB, MINB) dslash_tile_lc_kernel(const DslashKArgs a)
+// RPT right-hand sides per thread: block = 32 sites x RB / RPT warps
+template <int PREC, int RECON, int DAG, int RB, int MINB, int TPC, int RPT>
+__global__ void __launch_bounds__(32 * RB / RPT, MINB) dslash_tile_lc_kernel(const DslashKArgs a)
 {
+    static_assert(RB % RPT == 0, "right-hand sides per CTA must be a multiple of the right-hand sides per thread");
     constexpr int S = 32;
     constexpr uint32_t BYTES = (uint32_t)sizeof(TileSmem<S>);
     __shared__ __align__(128) TileSmem<S> sm[2];
@@ -645,8 +734,15 @@ __global__ void __launch_bounds__(32 * RB, MINB) dslash_tile_lc_kernel(const Dsl
     const int Vh = a.g.Vh, tiles = (Vh + S - 1) / S;
     const int tile0 = grp * TPC;
     const int ntile = min(TPC, tiles - tile0);
-    const int rhs = by * RB + ty;
-    const bool ract = rhs < a.nrhs && (a.active == nullptr || a.active[rhs] != 0);
+    const int rhs = by * RB + ty * RPT;
+    bool act[RPT];
+    bool ract = false, rall = true;
+#pragma unroll
+    for (int r = 0; r < RPT; ++r) {
+        act[r] = rhs + r < a.nrhs && (a.active == nullptr || a.active[rhs + r] != 0);
+        ract |= act[r];
+        rall &= act[r];
+    }
     const bool leader = (tx == 0 && ty == 0);
     const char* img = a.link_cache + ((size_t)a.parity * tiles + tile0) * sizeof(TileSmem<S>);
     if (leader) {
@@ -670,20 +766,32 @@ __global__ void __launch_bounds__(32 * RB, MINB) dslash_tile_lc_kernel(const Dsl
                 const int v = sm[b].nbr[d][tx];
                 nb[d] = v < 0 ? ~v : v;
             }
-            tile_site_any<PREC, RECON, DAG, 1>(a, sm[b], cb, tx, rhs, nb, 1.f, 1.f);
+            if constexpr (RPT == 1) {
+                tile_site_any<PREC, RECON, DAG, 1>(a, sm[b], cb, tx, rhs, nb, 1.f, 1.f);
+            } else {
+                if (rall) {
+                    tile_site_r<PREC, RECON, DAG, RPT>(a, sm[b], cb, tx, rhs, nb);
+                } else { // some right-hand sides of the group have converged: the others one at a time (same bits)
+                    for (int r = 0; r < RPT; ++r)
+                        if (act[r]) tile_site<PREC, RECON, DAG, 1>(a, sm[b], cb, tx, rhs + r, nb, 1.f, 1.f);
+                }
+            }
         }
         if (i + 1 < ntile) __syncthreads();
     }
 }
 
-template <int PREC, int RECON, int RB, int MINB, int TPC>
+#ifndef TM_LC_RPT
+#define TM_LC_RPT 1
+#endif
+template <int PREC, int RECON, int RB, int MINB, int TPC, int RPT = TM_LC_RPT>
 static inline void launch_tile_lc(const DslashKArgs& a, bool dagger, cudaStream_t st)
 {
     const int ny = (a.nrhs + RB - 1) / RB;
     const unsigned tiles = (unsigned)((a.g.Vh + 31) / 32);
-    dim3 block(32, RB), grid(((tiles + TPC - 1) / TPC) * ny);
-    if (dagger) dslash_tile_lc_kernel<PREC, RECON, 1, RB, MINB, TPC><<<grid, block, 0, st>>>(a);
-    else dslash_tile_lc_kernel<PREC, RECON, 0, RB, MINB, TPC><<<grid, block, 0, st>>>(a);
+    dim3 block(32, RB / RPT), grid(((tiles + TPC - 1) / TPC) * ny);
+    if (dagger) dslash_tile_lc_kernel<PREC, RECON, 1, RB, MINB, TPC, RPT><<<grid, block, 0, st>>>(a);
+    else dslash_tile_lc_kernel<PREC, RECON, 0, RB, MINB, TPC, RPT><<<grid, block, 0, st>>>(a);
 }
 
 template <int PREC, int RECON, int S, int RB, int MINB, int SL>

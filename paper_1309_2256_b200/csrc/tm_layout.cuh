@@ -288,7 +288,14 @@ __device__ __forceinline__ void load_link(const void* block, int Vh, int cb, typ
             unpack_w2<FX>(q.y, u[10], u[11]);
         }
     }
+#ifdef TM_DEBUG_NOREBUILD // timing ablation (probe builds only, wrong results): the third row is not rebuilt
+    if constexpr (RECON == 12) {
+#pragma unroll
+        for (int k = 0; k < 6; ++k) u[12 + k] = u[k];
+    }
+#else
     if constexpr (RECON == 12) rebuild_row2(u);
+#endif
 }
 
 } // namespace tmk

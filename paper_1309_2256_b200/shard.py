@@ -21,6 +21,37 @@ def owned_sources(n_sources, nrhs, rank, world):
     return [first + k for first, count in source_batches(n_sources, nrhs, rank, world) for k in range(count)]
 
 
+class LoopGather:
+    """The gather of gather_loops() with everything that does not depend on the data prepared once: block sizes, the padded
+    send block, the receive buffer and the index that puts the received rows into source order (one index_select per call,
+    no host-to-device copy and no synchronisation inside a timed loop)."""
+
+    def __init__(self, n_sources, nrhs, tail, dtype, device, group=None):
+        self.group = group
+        self.world = dist.get_world_size(group) if dist.is_initialized() else 1
+        self.rank = dist.get_rank(group) if dist.is_initialized() else 0
+        self.n_sources = n_sources
+        self.counts = [len(owned_sources(n_sources, nrhs, r, self.world)) for r in range(self.world)]
+        self.pad = max(self.counts) if self.counts else 0
+        tail = tuple(tail)
+        self.block = torch.zeros((self.pad,) + tail, dtype=dtype, device=device)
+        self.recv = torch.empty((self.world * self.pad,) + tail, dtype=dtype, device=device)
+        perm = [0] * n_sources
+        for r in range(self.world):
+            for k, src in enumerate(owned_sources(n_sources, nrhs, r, self.world)):
+                perm[src] = r * self.pad + k
+        self.perm = torch.tensor(perm, dtype=torch.long, device=device)
+
+    def __call__(self, local_loops):
+        if local_loops.shape[0] != self.counts[self.rank]:
+            raise ValueError("rank %d holds %d loops, owns %d sources" % (self.rank, local_loops.shape[0], self.counts[self.rank]))
+        if self.world == 1:
+            return local_loops.index_select(0, self.perm)
+        self.block[:self.counts[self.rank]] = local_loops
+        dist.all_gather_into_tensor(self.recv, self.block, group=self.group)
+        return self.recv.index_select(0, self.perm)
+
+
 def gather_loops(local_loops, n_sources, nrhs, group=None):
     """All ranks: local_loops[k] ([16][T][2] doubles) belongs to owned_sources(...)[k].  Returns [n_sources][16][T][2] in source
     order on every rank.  One all_gather of equally sized (padded) blocks."""
