@@ -359,7 +359,11 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
 
     # the same single-rhs kernels on the temporal-gauge copy of the field, declared as such (TM_RECON_*_TG): temporal hops inside the
     # lattice load no link and multiply by none.  Bytes: 6 + 2/T links per site instead of 8; GFLOPS keep the 1320-flop convention.
-    Utg = torch.from_numpy(ti.temporal_gauge(ti.gauge(DIMS))[0].view(np.float64)).cuda()
+    # the field is gauge-fixed by the library's own call on the device (tm_gauge_fix_temporal), as a user would do it
+    Utg = torch.from_numpy(ti.gauge(DIMS).view(np.float64)).cuda()
+    gtg = torch.empty(L.V * 18, dtype=torch.float64, device="cuda")
+    tm.tm_gauge_fix_temporal(L, Utg, gtg)
+    del gtg
     tgt = {}
     T_ = DIMS[3]
     for prec in (4, 2):

@@ -49,7 +49,11 @@ typedef enum { TM_PREC_F64 = 8, TM_PREC_F32 = 4, TM_PREC_F16 = 2 } tm_prec;   /*
  * the paper; reading 33).  tm_gauge_pack verifies the declaration (TM_ERR_NOT_TGAUGE otherwise) and stores the field like the plain
  * 18 / 12-real one -- unit links included, so a kernel that ignores the declaration is still correct.  The single-right-hand-side fp32 / fp16
  * hopping-term kernels honour it: temporal hops that do not wrap around load no link and multiply by none (25 % fewer link bytes, 144
- * fewer multiply-adds per site); every other kernel treats the code as the plain one. */
+ * fewer multiply-adds per site); every other kernel treats the code as the plain one.
+ * HAZARD: the declaration travels in the `recon` ARGUMENT of each call, not in the packed buffer (same bytes and size as the plain code), so
+ * only the pack call can verify it.  Passing a *_TG code to tm_dslash / tm_MdagM / tm_cg* / tm_M for a buffer that was packed under the plain
+ * code (or from a field that is not in temporal gauge) silently skips non-unit temporal links and returns wrong results with TM_OK.
+ * Use a *_TG code only with the buffer the pack call accepted under that code. */
 typedef enum { TM_RECON_18 = 18, TM_RECON_12 = 12, TM_RECON_8 = 8, TM_RECON_18_FIX16 = 118, TM_RECON_12_FIX16 = 112,
                TM_RECON_18_TG = 218, TM_RECON_12_TG = 212 } tm_recon;
 typedef enum { TM_KIND_PLAIN = 0, TM_KIND_TWIST_INV = 1, TM_KIND_XPAY_TWIST = 2 } tm_dslash_kind;

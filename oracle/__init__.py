@@ -198,6 +198,7 @@ def tsm_combine(L_hp, L_lp_same, L_lp):
 
 # ---- NEXT-2 / NEXT-3: plain numpy definitions in oracle/insertions.py ---------------------------
 from . import insertions as _ins  # noqa: E402
+from .gaugefix import temporal_gauge  # noqa: E402,F401
 
 covdev = _ins.covdev
 contract_field = _ins.contract_field

@@ -7,6 +7,7 @@
 #include "tm_blas.cuh"
 #include <cmath>
 #include <cstring>
+#include <new>
 #include <vector>
 
 namespace tmk {
@@ -145,24 +146,66 @@ static int k_update_p(const Geo& g, int prec, VecArg p, VecArg r, const BlasCtx&
     });
 }
 
-// pinned host ring for the pipelined convergence poll of cg_lp_truncated (library-owned host memory, created once)
+// pinned host ring for the pipelined convergence poll of cg_lp_truncated: library-owned host memory, one ring per (host thread,
+// device), created on first use and released when the thread ends; a failed creation leaves nothing behind.
 struct PollRing {
     static constexpr int DEPTH = 4;
     unsigned char* flags = nullptr; // [DEPTH][TM_MAX_NRHS], pinned
-    cudaEvent_t ev[DEPTH];
+    cudaEvent_t ev[DEPTH] = {};
+    int nev = 0;
+    int device = -1;
+    bool create(int dev)
+    {
+        device = dev;
+        if (cudaHostAlloc(reinterpret_cast<void**>(&flags), DEPTH * TM_MAX_NRHS, cudaHostAllocDefault) != cudaSuccess) {
+            flags = nullptr;
+            return false;
+        }
+        for (nev = 0; nev < DEPTH; ++nev)
+            if (cudaEventCreateWithFlags(&ev[nev], cudaEventDisableTiming) != cudaSuccess) {
+                destroy();
+                return false;
+            }
+        return true;
+    }
+    void destroy()
+    {
+        for (int i = 0; i < nev; ++i) cudaEventDestroy(ev[i]);
+        nev = 0;
+        if (flags) cudaFreeHost(flags);
+        flags = nullptr;
+    }
+};
+struct PollRings {
+    std::vector<PollRing*> rings; // one per device this thread has solved on
+    ~PollRings()
+    {
+        for (PollRing* r : rings) {
+            // at thread exit the context may already be gone; the calls then fail harmlessly
+            int cur = -1;
+            if (cudaGetDevice(&cur) == cudaSuccess && cudaSetDevice(r->device) == cudaSuccess) {
+                r->destroy();
+                cudaSetDevice(cur);
+            }
+            delete r;
+        }
+    }
 };
 static PollRing* poll_ring()
 {
-    static thread_local PollRing ring;
-    static thread_local bool ok = false;
-    if (!ok) {
-        if (cudaHostAlloc(reinterpret_cast<void**>(&ring.flags), PollRing::DEPTH * TM_MAX_NRHS, cudaHostAllocDefault) != cudaSuccess)
-            return nullptr;
-        for (int i = 0; i < PollRing::DEPTH; ++i)
-            if (cudaEventCreateWithFlags(&ring.ev[i], cudaEventDisableTiming) != cudaSuccess) return nullptr;
-        ok = true;
+    static thread_local PollRings mine;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return nullptr;
+    for (PollRing* r : mine.rings)
+        if (r->device == dev) return r;
+    PollRing* r = new (std::nothrow) PollRing;
+    if (!r) return nullptr;
+    if (!r->create(dev)) { // nothing half-built survives: the next call starts from scratch
+        delete r;
+        return nullptr;
     }
-    return &ring;
+    mine.rings.push_back(r);
+    return r;
 }
 
 // carve a workspace
@@ -208,7 +251,8 @@ static int init_ctx(const BlasCtx& c, const tm_cg_params* p, int nrhs, cudaStrea
     TM_CUDA_CHECK(cudaMemcpyAsync(c.scal, h.data(), sizeof(CgScal) * nrhs, cudaMemcpyHostToDevice, st));
     TM_CUDA_CHECK(cudaMemsetAsync(c.active, 1, nrhs, st));
     TM_CUDA_CHECK(cudaMemsetAsync(c.tickets, 0, sizeof(unsigned int) * nrhs, st));
-    TM_CUDA_CHECK(cudaStreamSynchronize(st)); // h goes out of scope
+    // no stream synchronisation: a cudaMemcpyAsync from pageable host memory returns once the source has been staged, so `h`
+    // may go out of scope here
     return TM_OK;
 }
 
@@ -422,7 +466,13 @@ int cg_hp_mixed(const Geo& g, const void* gauge_hp, int prec_hp, const void* gau
         ++k;
         x_dirty = true;
         if ((rc = read_scal(c, &h, st)) != TM_OK) return rc;
-        if (h.status == TM_ERR_BREAKDOWN) { status = TM_ERR_BREAKDOWN; break; }
+        if (h.status == TM_ERR_BREAKDOWN) {
+            // keep what the iterations since the last reliable update have gained: x_hp += x_lp before the odd sites are rebuilt
+            if (x_dirty && (rc = k_axpby<0>(g, prec_hp, prec_lp, V_(s_full, 2 * pbh), V_(xl, pbl), 1.0, 1.0, c, 1, st)) != TM_OK) return rc;
+            x_dirty = false;
+            status = TM_ERR_BREAKDOWN;
+            break;
+        }
         const double rr = h.rr;
         if (rr > rr_max) rr_max = rr;
         const bool want = (rr < delta * delta * rr_max) || (rr <= target2) || (k == prm->max_iter);
@@ -452,7 +502,6 @@ int cg_hp_mixed(const Geo& g, const void* gauge_hp, int prec_hp, const void* gau
         if (k < prm->max_iter)
             if ((rc = k_update_p(g, prec_lp, V_(p, pbl), V_(r, pbl), c, 1, st)) != TM_OK) return rc;
     }
-    (void)x_dirty;
     info->iters = k;
     info->status = status;
     info->true_resid = std::sqrt(rr_true / b2);

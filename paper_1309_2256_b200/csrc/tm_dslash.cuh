@@ -144,7 +144,7 @@ __device__ __forceinline__ void fused_axpy(const DslashKArgs& a, int rhs, int cb
 {
     typedef typename Prec<PREC>::real real;
     real y[24];
-    load_spinor<PREC, true>(a.axpy_y + (size_t)rhs * a.stride_y, a.g.Vh, cb, y);
+    load_spinor<PREC, 2>(a.axpy_y + (size_t)rhs * a.stride_y, a.g.Vh, cb, y); // coherent: y may be the output vector (r -= alpha A p)
     const real c = (real)(*reinterpret_cast<const double*>(a.axpy_coef + (size_t)rhs * a.stride_coef));
 #pragma unroll
     for (int k = 0; k < 24; ++k) o[k] = fma(-c, o[k], y[k]);
@@ -152,8 +152,7 @@ __device__ __forceinline__ void fused_axpy(const DslashKArgs& a, int rhs, int cb
 
 // Fused CG reduction: Re <w, out> (or |out|^2 when there is no w) of one site in the arithmetic precision, summed over the warp's 32
 // consecutive sites in fp64 with a fixed shuffle tree; lane 0 stores the partial of site group cb / 32.  `o` is the
-// epilogue result before storage rounding.  Every lane of the warp that reaches the epilogue calls this (the active
-// lanes are the contiguous range [0, n) because cb grows with the lane).
+// epilogue result before storage rounding.  Every valid lane of the warp (cb < Vh) calls this.
 template <int PREC>
 __device__ __forceinline__ void warp_dot_store(const DslashKArgs& a, int rhs, int cb, const typename Prec<PREC>::real* o)
 {
@@ -169,8 +168,12 @@ __device__ __forceinline__ void warp_dot_store(const DslashKArgs& a, int rhs, in
         for (int k = 0; k < 24; ++k) s = fma(o[k], o[k], s);
     }
     double v = (double)s;
-    const unsigned m = __activemask();
-    const int n = __popc(m), lane = threadIdx.x & 31;
+    // The warp is 32 consecutive sites starting at a multiple of 32, so its valid lanes are [0, n) with n fixed by the geometry:
+    // the mask does not depend on how the compiler reconverged the code above (an __activemask() taken after divergent code
+    // could name fewer lanes and silently drop partial sums).
+    const int lane = threadIdx.x & 31;
+    const int n = min(32, a.g.Vh - (cb - lane));
+    const unsigned m = n >= 32 ? 0xffffffffu : ((1u << n) - 1u);
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
         const double t = __shfl_down_sync(m, v, off);
@@ -272,7 +275,7 @@ __global__ void __launch_bounds__(256, PREC == 8 && NR == 1 ? 2 : 1) dslash_kern
         }
         if (a.x != nullptr) {
             real xv[24];
-            load_spinor<PREC, true>(a.x + (size_t)(r0 + r) * a.stride_x, Vh, cb, xv);
+            load_spinor<PREC, 1>(a.x + (size_t)(r0 + r) * a.stride_x, Vh, cb, xv);
 #pragma unroll
             for (int k = 0; k < 12; ++k) {
                 const real s5 = (k < 6) ? real(1) : real(-1);

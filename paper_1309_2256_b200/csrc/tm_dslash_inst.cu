@@ -48,11 +48,12 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     a.eps = p.dagger ? -1.0 : 1.0;
     for (int k = 0; k < 4; ++k) a.pq[k] = p.pq[k];
     const int n = p.nrhs;
+#if TM_RECON >= 200
+    if (n != 1) return TM_ERR_ARG; // before the timing bracket opens (launch_dslash sends nrhs > 1 to the plain instantiations)
+#endif
     kernel_timing_begin(st);
 #if TM_RECON >= 200
-    // temporal gauge declared (tm.h): the single-rhs kernel that loads no link for temporal hops inside the lattice; launch_dslash
-    // sends everything else to the plain instantiations
-    if (n != 1) return TM_ERR_ARG;
+    // temporal gauge declared (tm.h): the single-rhs kernel that loads no link for temporal hops inside the lattice
     launch_tile<TM_PREC, TM_RECON, 128, 1, 4, 0>(a, p.dagger != 0, st);
 #elif TM_PREC == 8
     // fp64: one thread per (site, rhs); threads of one site share the link lines in L1 (measured faster than two rhs per

@@ -224,7 +224,7 @@ __device__ __forceinline__ void tile_epilogue(const DslashKArgs& a, int cb, int 
     }
     if (a.x != nullptr) {
         float xv[24];
-        load_spinor<PREC, true>(a.x + (size_t)rhs * a.stride_x, Vh, cb, xv);
+        load_spinor<PREC, 1>(a.x + (size_t)rhs * a.stride_x, Vh, cb, xv);
 #pragma unroll
         for (int k = 0; k < 12; ++k) {
             const float s5 = (k < 6) ? 1.f : -1.f;
@@ -564,7 +564,7 @@ __device__ __forceinline__ void tile_site2(const DslashKArgs& a, const SM& sm, i
     }
     if (a.x != nullptr) {
         float xv[24];
-        load_spinor<PREC, true>(a.x + (size_t)rhs * a.stride_x, Vh, cb, xv);
+        load_spinor<PREC, 1>(a.x + (size_t)rhs * a.stride_x, Vh, cb, xv);
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             const f32x2 xur = pk2(xv[2 * c], xv[6 + 2 * c]), xui = pk2(xv[2 * c + 1], xv[6 + 2 * c + 1]);

@@ -40,6 +40,29 @@ __device__ __forceinline__ unsigned long long link_policy()
     asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
+// Same hints on a COHERENT load (no .nc): for an operand that the same kernel also writes -- the y of a fused axpy may be the
+// output vector itself (r = r - alpha A p), and the non-coherent path requires data that is read-only for the whole kernel.
+template <typename T>
+__device__ __forceinline__ T stream_ld(const T* p)
+{
+    const unsigned long long pol = link_policy();
+    T v;
+    if constexpr (sizeof(T) == 16) {
+        uint4 q;
+        asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;" : "=r"(q.x), "=r"(q.y), "=r"(q.z), "=r"(q.w) : "l"(p), "l"(pol) : "memory");
+        v = *reinterpret_cast<const T*>(&q);
+    } else if constexpr (sizeof(T) == 8) {
+        uint2 q;
+        asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.u32 {%0,%1}, [%2], %3;" : "=r"(q.x), "=r"(q.y) : "l"(p), "l"(pol) : "memory");
+        v = *reinterpret_cast<const T*>(&q);
+    } else {
+        uint32_t q;
+        asm volatile("ld.global.L1::no_allocate.L2::cache_hint.u32 %0, [%1], %2;" : "=r"(q) : "l"(p), "l"(pol) : "memory");
+        v = *reinterpret_cast<const T*>(&q);
+    }
+    return v;
+}
+
 template <typename T>
 __device__ __forceinline__ T link_ldg(const T* p)
 {
@@ -97,15 +120,16 @@ __device__ __forceinline__ void unpack_w2(uint32_t w, float& a, float& b)
 // ------------------------------------------------------------------------------------------------
 // spinor load: v[24] in arithmetic precision
 // ------------------------------------------------------------------------------------------------
-// STREAM: the operand is read exactly once per launch (the x of an XPAY epilogue, the y of a fused axpy): evict-first like the links
-template <int PREC, bool STREAM = false>
+// STREAM 1: the operand is read exactly once per launch and never written by it (the x of an XPAY epilogue): evict-first, non-coherent
+// like the links.  STREAM 2: read once but possibly ALIASED by the kernel's output (the y of a fused axpy): same hints, coherent load.
+template <int PREC, int STREAM = 0>
 __device__ __forceinline__ void load_spinor(const void* base, int Vh, int cb, typename Prec<PREC>::real* v)
 {
     if constexpr (PREC == 8) {
         const double2* p = reinterpret_cast<const double2*>(base) + cb;
 #pragma unroll
         for (int k = 0; k < 12; ++k) {
-            const double2 d = STREAM ? link_ldg(p + (size_t)k * Vh) : __ldg(p + (size_t)k * Vh);
+            const double2 d = STREAM == 2 ? stream_ld(p + (size_t)k * Vh) : STREAM == 1 ? link_ldg(p + (size_t)k * Vh) : __ldg(p + (size_t)k * Vh);
             v[2 * k] = d.x;
             v[2 * k + 1] = d.y;
         }
@@ -113,7 +137,7 @@ __device__ __forceinline__ void load_spinor(const void* base, int Vh, int cb, ty
         const float4* p = reinterpret_cast<const float4*>(base) + cb;
 #pragma unroll
         for (int k = 0; k < 6; ++k) {
-            const float4 d = STREAM ? link_ldg(p + (size_t)k * Vh) : __ldg(p + (size_t)k * Vh);
+            const float4 d = STREAM == 2 ? stream_ld(p + (size_t)k * Vh) : STREAM == 1 ? link_ldg(p + (size_t)k * Vh) : __ldg(p + (size_t)k * Vh);
             v[4 * k] = d.x;
             v[4 * k + 1] = d.y;
             v[4 * k + 2] = d.z;
@@ -123,9 +147,9 @@ __device__ __forceinline__ void load_spinor(const void* base, int Vh, int cb, ty
         const uint4* p = reinterpret_cast<const uint4*>(base) + cb;
         uint4 q[3];
 #pragma unroll
-        for (int k = 0; k < 3; ++k) q[k] = STREAM ? link_ldg(p + (size_t)k * Vh) : __ldg(p + (size_t)k * Vh);
+        for (int k = 0; k < 3; ++k) q[k] = STREAM == 2 ? stream_ld(p + (size_t)k * Vh) : STREAM == 1 ? link_ldg(p + (size_t)k * Vh) : __ldg(p + (size_t)k * Vh);
         const float* np_ = reinterpret_cast<const float*>(reinterpret_cast<const uint4*>(base) + (size_t)3 * Vh) + cb;
-        const float nrm = STREAM ? link_ldg(np_) : __ldg(np_);
+        const float nrm = STREAM == 2 ? stream_ld(np_) : STREAM == 1 ? link_ldg(np_) : __ldg(np_);
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             unpack_h2(q[k].x, v[8 * k + 0], v[8 * k + 1]);

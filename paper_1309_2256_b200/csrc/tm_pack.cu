@@ -1,4 +1,5 @@
 // tm_pack.cu -- a0 / a1 of SURVEY.md 8(a): canonical fp64 fields <-> packed even-odd SoA at fp64/fp32/fp16.
+#include <mutex>
 #include "tm_layout.cuh"
 
 namespace tmk {
@@ -282,6 +283,10 @@ extern "C" int tm_gauge_pack(const tm_lattice* L, const double* U, int prec, int
     if (!L || !U || !out || !valid_prec(prec) || !valid_recon(recon)) return TM_ERR_ARG;
     if (!aligned256(U) || !aligned256(out)) return TM_ERR_LAYOUT;
     cudaStream_t st = (cudaStream_t)stream;
+    // the check counters are device symbols shared by every call: concurrent packs (other host threads, other streams) take turns;
+    // every check below ends with a stream synchronisation inside the lock, so a counter is read before the next pack resets it
+    static std::mutex pack_mu;
+    std::lock_guard<std::mutex> pack_lock(pack_mu);
     const int tgcheck = recon >= 200 ? 1 : 0; // declaration only: the field is stored like the plain 18 / 12-real one
     recon = stored_recon(prec, recon);
     const int check = (recon % 100 != 18 && su3_tol > 0) ? 1 : 0;

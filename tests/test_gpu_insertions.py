@@ -147,7 +147,7 @@ def test_hpe_remainder(prec, recon):
     tm.tm_hpe_remainder(F.L, F.gauge(prec, recon), prec, recon, out, ps, tmp, KAPPA, MU, 2)
     got = F.unpack(out, prec, nrhs=2)
     for r in range(2):
-        assert rel(got[r], oracle.hpe_remainder(U, s[r], KAPPA, MU)) < (4 if prec == 2 else 1) * TOL[prec]
+        assert rel(got[r], oracle.hpe_remainder(U, s[r], KAPPA, MU)) < TOL[prec]  # measured 5.6e-4 (fp16) / 2.0e-7 (fp32) at 32^3x64: DESIGN.md reading 34
 
 
 def test_hpe_estimator_exact_on_4x4():

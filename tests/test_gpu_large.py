@@ -202,4 +202,8 @@ def test_32x64_insertions_full_size(prec):
     # hopping-parameter remainder
     tmp = F.zeros_full(prec)
     tm.tm_hpe_remainder(F.L, F.gauge(prec, 12), prec, 12, d, pb_, tmp, KAPPA, MU, 1)
-    assert rel(F.unpack(d, prec), oracle.hpe_remainder(U, b, KAPPA, MU)) < (4 if prec == 2 else 1) * TOL[prec]
+    err = rel(F.unpack(d, prec), oracle.hpe_remainder(U, b, KAPPA, MU))
+    print("(BH)^4 relative L2 error at 32^3x64, storage bytes %d: %.3e" % (prec, err))
+    # eight launches in a row, each rounding its result to the storage format; measured 5.6e-4 (fp16 storage) and 2.0e-7 (fp32)
+    # on this field: the single-launch bound holds with room to spare (reading 34)
+    assert err < TOL[prec]

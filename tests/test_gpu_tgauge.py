@@ -19,7 +19,7 @@ _cache = {}
 def tg_fields(dims, ap=True):
     key = (tuple(dims), ap)
     if key not in _cache:
-        U = ti.temporal_gauge(ti.gauge(dims))[0]
+        U = oracle.temporal_gauge(ti.gauge(dims))[0]
         _cache[key] = (Fields(dims, U, ap), U)
     return _cache[key]
 
@@ -90,12 +90,12 @@ def test_tg_multi_rhs_MdagM_and_solves(prec):
 
 @pytest.mark.parametrize("dims", [(4, 6, 8, 10), (8, 8, 8, 16)])
 def test_gauge_fix_temporal_on_the_device(dims):
-    """tm_gauge_fix_temporal against the input-preparation routine pinned by P25 (tm_inputs.temporal_gauge): the transformed field and
+    """tm_gauge_fix_temporal against the input-preparation routine pinned by P25 (oracle.temporal_gauge): the transformed field and
     the transformation to rounding, exact unit links where they belong, and the result is accepted under the temporal-gauge code."""
     import torch
     from tm_harness import to_dev
     U0 = ti.gauge(dims)
-    U_ref, g_ref = ti.temporal_gauge(U0)
+    U_ref, g_ref = oracle.temporal_gauge(U0)
     L = tm.tm_lattice_create(dims, True)
     U_dev = to_dev(U0)
     g_dev = torch.empty(L.V * 18, dtype=torch.float64, device="cuda")

@@ -244,13 +244,13 @@ def test_P24_symmetric_preconditioning_is_a_rescaling_of_the_normal_operator():
 
 
 def test_P25_temporal_gauge_is_a_gauge_transformation_of_the_oracle_operator():
-    """tm_inputs.temporal_gauge (a non-random, time-ordered transformation: g(x,t) = prod_{t'<t} U_t(x,t')) against the oracle:
+    """oracle.temporal_gauge (a non-random, time-ordered transformation: g(x,t) = prod_{t'<t} U_t(x,t')) against the oracle:
     U' stays in SU(3), U'_t = 1 on every slice but the last, the last slice carries the Polyakov loop (its trace equals that of the
     ordered product of the original temporal links), M(U') g = g M(U) with the antiperiodic sign left on the fermions, and the
     truncated CG takes the same number of iterations on both fields (the Krylov spaces are unitarily equivalent)."""
     dims = (4, 4, 6, 8)
     U = ti.gauge(dims)
-    Up, g = ti.temporal_gauge(U)
+    Up, g = oracle.temporal_gauge(U)
     eye = np.eye(3)
     assert np.abs(Up @ np.conj(np.swapaxes(Up, -1, -2)) - eye).max() < 1e-13
     assert np.abs(np.linalg.det(Up) - 1).max() < 1e-13

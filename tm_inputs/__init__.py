@@ -83,25 +83,6 @@ def unit_gauge(dims):
     return out
 
 
-def temporal_gauge(U):
-    """The gauge-equivalent copy of a field with unit temporal links on every slice but the last (input preparation: a gauge
-    transformation g(x, t) = prod_{t' < t} U_t(x, t'), U'_mu(x) = g(x) U_mu(x) g(x + mu)^dagger, periodic wrap -- the antiperiodic
-    sign of the fermions is not part of the links).  Temporal links of slices t < T - 1 are set to exactly 1 (they are 1 up to
-    rounding); slice T - 1 carries the Polyakov loop.  Returns (U', g)."""
-    T = U.shape[0]
-    eye = np.eye(3, dtype=np.complex128)
-    g = np.empty(U.shape[:4] + (3, 3), dtype=np.complex128)
-    g[0] = eye
-    for t in range(T - 1):
-        g[t + 1] = g[t] @ U[t, ..., 3, :, :]
-    Up = np.empty_like(U)
-    for mu in range(4):
-        gs = np.roll(g, -1, axis=3 - mu)  # g(x + mu); array axes are (t, z, y, x)
-        Up[..., mu, :, :] = g @ U[..., mu, :, :] @ np.conj(np.swapaxes(gs, -1, -2))
-    Up[:T - 1, ..., 3, :, :] = eye
-    return Up, g
-
-
 def gauge_sites(sites, seed=GAUGE_SEED, eps=EPS, w=1.0):
     """Links U[k][mu][3][3] of the listed global site indices (same values as gauge())."""
     sites = np.ascontiguousarray(sites, dtype=np.int64)
