@@ -75,10 +75,10 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     else if (a.link_cache) {
         static const int cfg = getenv("TM_LC_CFG") ? atoi(getenv("TM_LC_CFG")) : 0;
         switch (cfg) {
-#define TM_CASE(id, RB, MINB, TPC, RPT) case id: launch_tile_lc<TM_PREC, TM_RECON, RB, MINB, TPC, RPT>(a, dg, st); break;
+#define TM_CASE(id, RB, MINB, TPC) case id: launch_tile_lc<TM_PREC, TM_RECON, RB, MINB, TPC>(a, dg, st); break;
             TM_SWEEP_CASES
 #undef TM_CASE
-        default: launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 4, 1>(a, dg, st);
+        default: launch_tile_lc<TM_PREC, TM_RECON, 12, 2, 4>(a, dg, st);
         }
     }
 #else
@@ -98,7 +98,7 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
 #define TM_STR(x) TM_STR2(x)
 const char* lc_kernel_signature()
 {
-    return "dslash_tile_lc_kernel<prec=2,recon=12,RB=" TM_STR(TM_LC_RB) ",MINB=" TM_STR(TM_LC_MINB) ",TPC=" TM_STR(TM_LC_TPC) ",RPT=" TM_STR(TM_LC_RPT) ">";
+    return "dslash_tile_lc_kernel<prec=2,recon=12,RB=" TM_STR(TM_LC_RB) ",MINB=" TM_STR(TM_LC_MINB) ",TPC=" TM_STR(TM_LC_TPC) ">";
 }
 #endif
 

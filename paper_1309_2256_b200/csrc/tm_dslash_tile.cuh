@@ -322,65 +322,6 @@ __device__ __forceinline__ void tile_site(const DslashKArgs& a, const SM& sm, in
     tile_epilogue<PREC>(a, cb, rhs, acc);
 }
 
-// ---- R right-hand sides per thread (multi-rhs kernels) -------------------------------------------------------
-// One thread owns a site and walks R right-hand sides inside the direction loop: the direction's 18 link reals are read
-// from the tile image ONCE and stay in registers for the R SU(3) products (4.5 LDS per R hops instead of per hop), the
-// neighbour index and its address arithmetic are shared, and the R gathers of a direction are in flight together.
-// Scalar FFMA with the operation order of tile_site, so every right-hand side gets the bits it gets alone.
-template <int PREC, int MUD, int E>
-__device__ __forceinline__ void tile_hop_acc(const Raw<PREC>& cur, const float* u, float* acc)
-{
-    float h[12], g[12];
-    float w = 1.f;
-    if constexpr (PREC == 2) w = cur.nrm;
-    tile_project<PREC, MUD, E>(cur, h);
-    su3_mul<0>(u, h, g);
-    tile_reconstruct<MUD, E, true>(acc, g, w);
-}
-
-template <int PREC, int RECON, int DAG, int R, typename SM>
-__device__ __forceinline__ void tile_site_r(const DslashKArgs& a, const SM& sm, int cb, int tx, int rhs0, const int* nb)
-{
-    constexpr int E = DAG ? -1 : 1;
-    const int Vh = a.g.Vh;
-    float acc[R][24];
-#pragma unroll
-    for (int r = 0; r < R; ++r)
-#pragma unroll
-        for (int k = 0; k < 24; ++k) acc[r][k] = 0.f;
-#pragma unroll
-    for (int d = 0; d < 8; ++d) {
-        Raw<PREC> cur[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) load_raw<PREC>(a.in + (size_t)(rhs0 + r) * a.stride_in, Vh, nb[d], cur[r]);
-        float u[18];
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const float4 q = sm.u4[d][k][tx];
-            u[4 * k] = q.x;
-            u[4 * k + 1] = q.y;
-            u[4 * k + 2] = q.z;
-            u[4 * k + 3] = q.w;
-        }
-        const float2 q2 = sm.u2[d][tx];
-        u[16] = q2.x;
-        u[17] = q2.y;
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            if (d == 0) tile_hop_acc<PREC, 0, E>(cur[r], u, acc[r]);
-            if (d == 1) tile_hop_acc<PREC, 0, -E>(cur[r], u, acc[r]);
-            if (d == 2) tile_hop_acc<PREC, 1, E>(cur[r], u, acc[r]);
-            if (d == 3) tile_hop_acc<PREC, 1, -E>(cur[r], u, acc[r]);
-            if (d == 4) tile_hop_acc<PREC, 2, E>(cur[r], u, acc[r]);
-            if (d == 5) tile_hop_acc<PREC, 2, -E>(cur[r], u, acc[r]);
-            if (d == 6) tile_hop_acc<PREC, 3, E>(cur[r], u, acc[r]);
-            if (d == 7) tile_hop_acc<PREC, 3, -E>(cur[r], u, acc[r]);
-        }
-    }
-#pragma unroll
-    for (int r = 0; r < R; ++r) tile_epilogue<PREC>(a, cb, rhs0 + r, acc[r]);
-}
-
 // ---- packed fp32x2 variant of phase B ----------------------------------------------------------------
 // sm_100a issues `fma.rn.f32x2` (SASS FFMA2: two fp32 FMAs on a 64-bit register pair, one issue slot, scalar operands
 // broadcast and negated as modifiers).  The two spin components of a projected half spinor are multiplied by the SAME
@@ -718,11 +659,9 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
                  : "memory");
 }
 
-// RPT right-hand sides per thread: block = 32 sites x RB / RPT warps
-template <int PREC, int RECON, int DAG, int RB, int MINB, int TPC, int RPT>
-__global__ void __launch_bounds__(32 * RB / RPT, MINB) dslash_tile_lc_kernel(const DslashKArgs a)
+template <int PREC, int RECON, int DAG, int RB, int MINB, int TPC>
+__global__ void __launch_bounds__(32 * RB, MINB) dslash_tile_lc_kernel(const DslashKArgs a)
 {
-    static_assert(RB % RPT == 0, "right-hand sides per CTA must be a multiple of the right-hand sides per thread");
     constexpr int S = 32;
     constexpr uint32_t BYTES = (uint32_t)sizeof(TileSmem<S>);
     __shared__ __align__(128) TileSmem<S> sm[2];
@@ -734,15 +673,8 @@ __global__ void __launch_bounds__(32 * RB / RPT, MINB) dslash_tile_lc_kernel(con
     const int Vh = a.g.Vh, tiles = (Vh + S - 1) / S;
     const int tile0 = grp * TPC;
     const int ntile = min(TPC, tiles - tile0);
-    const int rhs = by * RB + ty * RPT;
-    bool act[RPT];
-    bool ract = false, rall = true;
-#pragma unroll
-    for (int r = 0; r < RPT; ++r) {
-        act[r] = rhs + r < a.nrhs && (a.active == nullptr || a.active[rhs + r] != 0);
-        ract |= act[r];
-        rall &= act[r];
-    }
+    const int rhs = by * RB + ty;
+    const bool ract = rhs < a.nrhs && (a.active == nullptr || a.active[rhs] != 0);
     const bool leader = (tx == 0 && ty == 0);
     const char* img = a.link_cache + ((size_t)a.parity * tiles + tile0) * sizeof(TileSmem<S>);
     if (leader) {
@@ -752,7 +684,8 @@ __global__ void __launch_bounds__(32 * RB / RPT, MINB) dslash_tile_lc_kernel(con
     }
     if (__syncthreads_or(ract) == 0) return;
     if (leader) bulk_load(smem_u32(&sm[0]), img, BYTES, smem_u32(&bar[0]));
-    // (decoupling the warps with per-buffer "empty" mbarriers instead of the CTA barrier was measured 2 % slower)
+    // (decoupling the warps with per-buffer "empty" mbarriers instead of the CTA barrier was measured 2 % slower; two to six
+    // right-hand sides per thread with the links kept in registers 15 % to 4.8 x slower: profiles/r02_ablations_12rhs_dslash.md)
     for (int i = 0; i < ntile; ++i) {
         const int b = i & 1;
         if (leader && i + 1 < ntile) // buffer b^1 was released by the barrier that closed tile i-1
@@ -766,32 +699,20 @@ __global__ void __launch_bounds__(32 * RB / RPT, MINB) dslash_tile_lc_kernel(con
                 const int v = sm[b].nbr[d][tx];
                 nb[d] = v < 0 ? ~v : v;
             }
-            if constexpr (RPT == 1) {
-                tile_site_any<PREC, RECON, DAG, 1>(a, sm[b], cb, tx, rhs, nb, 1.f, 1.f);
-            } else {
-                if (rall) {
-                    tile_site_r<PREC, RECON, DAG, RPT>(a, sm[b], cb, tx, rhs, nb);
-                } else { // some right-hand sides of the group have converged: the others one at a time (same bits)
-                    for (int r = 0; r < RPT; ++r)
-                        if (act[r]) tile_site<PREC, RECON, DAG, 1>(a, sm[b], cb, tx, rhs + r, nb, 1.f, 1.f);
-                }
-            }
+            tile_site_any<PREC, RECON, DAG, 1>(a, sm[b], cb, tx, rhs, nb, 1.f, 1.f);
         }
         if (i + 1 < ntile) __syncthreads();
     }
 }
 
-#ifndef TM_LC_RPT
-#define TM_LC_RPT 1
-#endif
-template <int PREC, int RECON, int RB, int MINB, int TPC, int RPT = TM_LC_RPT>
+template <int PREC, int RECON, int RB, int MINB, int TPC>
 static inline void launch_tile_lc(const DslashKArgs& a, bool dagger, cudaStream_t st)
 {
     const int ny = (a.nrhs + RB - 1) / RB;
     const unsigned tiles = (unsigned)((a.g.Vh + 31) / 32);
-    dim3 block(32, RB / RPT), grid(((tiles + TPC - 1) / TPC) * ny);
-    if (dagger) dslash_tile_lc_kernel<PREC, RECON, 1, RB, MINB, TPC, RPT><<<grid, block, 0, st>>>(a);
-    else dslash_tile_lc_kernel<PREC, RECON, 0, RB, MINB, TPC, RPT><<<grid, block, 0, st>>>(a);
+    dim3 block(32, RB), grid(((tiles + TPC - 1) / TPC) * ny);
+    if (dagger) dslash_tile_lc_kernel<PREC, RECON, 1, RB, MINB, TPC><<<grid, block, 0, st>>>(a);
+    else dslash_tile_lc_kernel<PREC, RECON, 0, RB, MINB, TPC><<<grid, block, 0, st>>>(a);
 }
 
 template <int PREC, int RECON, int S, int RB, int MINB, int SL>
