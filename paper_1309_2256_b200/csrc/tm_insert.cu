@@ -10,8 +10,11 @@
 //   tm_hpe_remainder     (B H)^4 s, B = R^-1, H = -kappa Dslash: the stochastic term of Eq. (17)
 //   tm_hpe_local_traces  per-site Tr[Gamma_n (B - BHB + (BH)^2 B - (BH)^3 B)]_xx, the exact terms of Eq. (16) for ultra-local X
 // (tm_loop_contract_slice, the single-time-slice contraction, lives in tm_loop.cu.)
+#include <cmath>
+#include <cstring>
 #include "tm_dslash_tile.cuh"
 #include "tm_gamma.cuh"
+#include "tm_contract.cuh"
 
 namespace tmk {
 
@@ -308,20 +311,163 @@ __global__ void __launch_bounds__(MOM_THREADS, PREC == 8 ? 2 : 3) loop_mom_plane
     }
 }
 
+// ---- stage 1 for fp32 / fp16 fields, X <= 64, Y <= 128: one warp per row, no CTA barrier inside the plane ----------------------
+// CTA = one (z, t) plane of one right-hand side, warp w = the rows y in [8 w, 8 w + 8).  Per row:
+//   (1) lane = site x: colour-traced contraction C[32 reals] (fp16 fields: exact products of the stored words, FHFMA) into a
+//       warp-private shared-memory tile [x][33];
+//   (2) lane = one of the 32 reals k = (ab, re/im): sums over x with REAL weights, even / odd split in x -> X - x (cos is even,
+//       sin is odd: half the multiplies): Sc[n] = sum C cos(n th x), Ss[n] = sum C sin(n th x), n <= P; the weights are warp
+//       uniform and come from the kernel parameters (constant bank), not from shared memory;
+//   (3) sums over y into (2P+1)^2 fp32 registers per lane (at most 8 rows, the LOOP_CHUNK rule of the loop kernel).
+// The warps' partials are then added in fp64 in a fixed order and turned into W2[ipx][ipy][ab] (the layout stage 2 reads).
+struct MomWeights {
+    float xc[MOM_MAXP + 1][32];            // cos(2 pi n j / X), j < X/2
+    float xs[MOM_MAXP + 1][32];            // sin(2 pi n j / X)
+    float yw[128][2 * MOM_MAXP + 1];       // row y: cos(2 pi m y / Y), m = 0..P, then sin(2 pi m y / Y), m = 1..P
+};
+constexpr int MOMR_ROWS = 8; // rows per warp
+// CTAs per SM asked of the compiler for the 4-warp shape (B200 sweep at 32^3 x 64, 12 sources, 123 momenta): fp16 storage 1122 / 1022 /
+// 986 / 1082 us at 4 / 5 / 6 / 8, fp32 1163 / 1215 / 1213 / 1587 us
+template <int PREC> struct MomrMinb { static constexpr int value = PREC == 2 ? 6 : 4; };
+
+// XH: X / 2 as a compile-time constant (the x loop is unrolled: tile reads and weights become immediates), 0 = run-time X.
+// MAXT / MINB: launch bounds (threads per CTA = 32 x ceil(Y / 8)).
+template <int PREC, int P, int XH, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) loop_mom_row_kernel(Geo g, const char* a_full, const char* b_full, size_t parity_bytes,
+                                                                  const __grid_constant__ MomWeights W, double2* W2)
+{
+    constexpr int NX = 2 * P + 1;
+    extern __shared__ float msm[];
+    const int X = XH ? 2 * XH : g.X, Y = g.Y, XT = X > 32 ? 64 : 32;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    float* tile = msm + (size_t)warp * XT * 33; // [x][33]
+    float* part = msm + (size_t)warp * NX * NX * 32; // [xi][yi][k]; written after every warp is done with its tile
+    const int z = blockIdx.x, t = blockIdx.y, rhs = blockIdx.z;
+    const char* af = a_full + (size_t)rhs * 2 * parity_bytes;
+    const char* bf = b_full + (size_t)rhs * 2 * parity_bytes;
+    float acc[NX][NX];
+#pragma unroll
+    for (int i = 0; i < NX; ++i)
+#pragma unroll
+        for (int j = 0; j < NX; ++j) acc[i][j] = 0.f;
+    const int y1 = min(Y, (warp + 1) * MOMR_ROWS);
+    for (int y = warp * MOMR_ROWS; y < y1; ++y) {
+        // (1) contraction of the row
+        for (int x = lane; x < X; x += 32) {
+            const int parity = (x + y + z + t) & 1;
+            const int cb = (x >> 1) + g.Xh * (y + Y * (z + g.Z * t));
+            float c[32];
+            if constexpr (PREC == 2) {
+                uint4 qa[3], qb[3];
+                const uint4* pa = reinterpret_cast<const uint4*>(af + (size_t)parity * parity_bytes) + cb;
+                const uint4* pb = reinterpret_cast<const uint4*>(bf + (size_t)parity * parity_bytes) + cb;
+#pragma unroll
+                for (int k = 0; k < 3; ++k) {
+                    qa[k] = __ldg(pa + (size_t)k * g.Vh);
+                    qb[k] = __ldg(pb + (size_t)k * g.Vh);
+                }
+                const float na = __ldg(reinterpret_cast<const float*>(reinterpret_cast<const uint4*>(af + (size_t)parity * parity_bytes) + (size_t)3 * g.Vh) + cb);
+                const float nb_ = __ldg(reinterpret_cast<const float*>(reinterpret_cast<const uint4*>(bf + (size_t)parity * parity_bytes) + (size_t)3 * g.Vh) + cb);
+#pragma unroll
+                for (int k = 0; k < 32; ++k) c[k] = 0.f;
+                site_contract_h(qa, na, qb, nb_, c);
+            } else {
+                float a[24], b[24];
+                load_spinor<PREC>(af + (size_t)parity * parity_bytes, g.Vh, cb, a);
+                load_spinor<PREC>(bf + (size_t)parity * parity_bytes, g.Vh, cb, b);
+                site_contract<float>(a, b, c);
+            }
+#pragma unroll
+            for (int k = 0; k < 32; ++k) tile[x * 33 + k] = c[k];
+        }
+        __syncwarp();
+        // (2) sums over x for the real k = lane
+        float S[NX];
+        {
+            const float e0 = tile[lane], eh = tile[(X >> 1) * 33 + lane];
+#pragma unroll
+            for (int n = 0; n <= P; ++n) S[n] = (n & 1) ? e0 - eh : e0 + eh;
+#pragma unroll
+            for (int n = 1; n <= P; ++n) S[P + n] = 0.f;
+#pragma unroll
+            for (int j = 1; j < (XH ? XH : (X >> 1)); ++j) {
+                const float cj = tile[j * 33 + lane], cm = tile[(X - j) * 33 + lane];
+                const float e = cj + cm, o = cj - cm;
+                S[0] += e;
+#pragma unroll
+                for (int n = 1; n <= P; ++n) {
+                    S[n] = fmaf(e, W.xc[n][j], S[n]);
+                    S[P + n] = fmaf(o, W.xs[n][j], S[P + n]);
+                }
+            }
+        }
+        __syncwarp(); // the tile is free for the next row
+        // (3) sums over y
+#pragma unroll
+        for (int yi = 0; yi < NX; ++yi) {
+            const float wy = yi == 0 ? 1.f : W.yw[y][yi];
+#pragma unroll
+            for (int xi = 0; xi < NX; ++xi) acc[xi][yi] = yi == 0 ? acc[xi][yi] + S[xi] : fmaf(S[xi], wy, acc[xi][yi]);
+        }
+    }
+    __syncthreads(); // the partials alias the tiles
+#pragma unroll
+    for (int xi = 0; xi < NX; ++xi)
+#pragma unroll
+        for (int yi = 0; yi < NX; ++yi) part[(xi * NX + yi) * 32 + lane] = acc[xi][yi];
+    __syncthreads();
+    // combine: item = (ipx, ipy, ab); A(xi, yi, k) = sum over the warps in fp64, fixed order
+    const float* part0 = msm;
+    double2* dst = W2 + (((size_t)rhs * g.T + t) * g.Z + z) * (NX * NX * 16);
+    for (int item = threadIdx.x; item < NX * NX * 16; item += blockDim.x) {
+        const int ab = item & 15, ipy = (item >> 4) % NX, ipx = (item >> 4) / NX;
+        const int nx = ipx - P, ny = ipy - P, ax = nx < 0 ? -nx : nx, ay = ny < 0 ? -ny : ny;
+        const double sx = nx > 0 ? 1.0 : (nx < 0 ? -1.0 : 0.0), sy = ny > 0 ? 1.0 : (ny < 0 ? -1.0 : 0.0);
+        double v[4][2]; // (cc, cs, sc, ss) x (re, im)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int xi = (q & 2) ? P + ax : ax, yi = (q & 1) ? P + ay : ay;
+            const bool on = !((q & 2) && ax == 0) && !((q & 1) && ay == 0);
+#pragma unroll
+            for (int ri = 0; ri < 2; ++ri) {
+                double sum = 0.0;
+                if (on)
+                    for (int w = 0; w < nwarp; ++w) sum += (double)part0[((size_t)w * NX * NX + (xi * NX + yi)) * 32 + 2 * ab + ri];
+                v[q][ri] = sum;
+            }
+        }
+        // sum C (cos_x - i sx sin_x)(cos_y - i sy sin_y), C = Cr + i Ci
+        const double re = v[0][0] - sx * sy * v[3][0] + (sy * v[1][1] + sx * v[2][1]);
+        const double im = v[0][1] - sx * sy * v[3][1] - (sy * v[1][0] + sx * v[2][0]);
+        dst[(ipx * NX + ipy) * 16 + ab] = make_double2(re, im);
+    }
+}
+
 // out[rhs][n][t][k] = sum_ab (Gamma_n)_ab sum_z e^{-2 pi i n_z z / Z} W2[rhs][t][z][ipx_k][ipy_k][ab]; 8 momenta per CTA
 __global__ void __launch_bounds__(128) loop_mom_final_kernel(Geo g, int P, const double2* W2, const int* mom, int K, GammaTable tb,
                                                              double* out)
 {
     __shared__ double2 Ck[8][16];
+    __shared__ double2 ph[256]; // e^{-2 pi i m / Z}, m < Z (Z <= 256; larger Z evaluates the phase per term)
     const int t = blockIdx.x, rhs = blockIdx.y;
     const int NP = 2 * P + 1, nout = NP * NP * 16;
     const int kk = threadIdx.x >> 4, ab = threadIdx.x & 15;
     const int k = blockIdx.z * 8 + kk;
+    const bool table = g.Z <= 256;
+    if (table)
+        for (int m = threadIdx.x; m < g.Z; m += blockDim.x) ph[m] = dft_phase(1, m, g.Z);
+    __syncthreads();
     if (k < K) {
         const int nx = mom[3 * k], ny = mom[3 * k + 1], nz = mom[3 * k + 2];
         const double2* src = W2 + ((size_t)rhs * g.T + t) * g.Z * nout + ((nx + P) * NP + (ny + P)) * 16 + ab;
         double2 s = make_double2(0.0, 0.0);
-        for (int z = 0; z < g.Z; ++z) s = cfma(src[(size_t)z * nout], dft_phase(nz, z, g.Z), s);
+        int m = 0;                                   // (nz z) mod Z, stepped
+        const int step = ((nz % g.Z) + g.Z) % g.Z;
+        for (int z = 0; z < g.Z; ++z) {
+            s = cfma(src[(size_t)z * nout], table ? ph[m] : dft_phase(nz, z, g.Z), s);
+            m += step;
+            if (m >= g.Z) m -= g.Z;
+        }
         Ck[kk][ab] = s;
     }
     __syncthreads();
@@ -490,6 +636,55 @@ extern "C" int tm_loop_momentum(const tm_lattice* L, const void* a_full, const v
     TM_CUDA_CHECK(cudaMemcpyAsync(mom_dev, momenta, (size_t)n_momenta * 3 * sizeof(int), cudaMemcpyHostToDevice, st));
     const size_t pb = spinor_parity_bytes(g, prec);
     dim3 grid(g.Z, g.T, nrhs);
+    if (prec != 8 && g.X <= 64 && g.Y <= 128) {
+        // fp32 / fp16 fields: warp-per-row kernel (no CTA barrier inside a plane, weights in the constant bank)
+        MomWeights w;
+        memset(&w, 0, sizeof(w));
+        const double pi2 = 6.283185307179586476925286766559;
+        for (int n = 0; n <= P; ++n)
+            for (int j = 0; j < g.X / 2; ++j) {
+                w.xc[n][j] = (float)cos(pi2 * ((n * j) % g.X) / g.X);
+                w.xs[n][j] = (float)sin(pi2 * ((n * j) % g.X) / g.X);
+            }
+        for (int y = 0; y < g.Y; ++y)
+            for (int m = 0; m <= P; ++m) {
+                w.yw[y][m] = (float)cos(pi2 * ((m * y) % g.Y) / g.Y);
+                if (m > 0) w.yw[y][P + m] = (float)sin(pi2 * ((m * y) % g.Y) / g.Y);
+            }
+        const int nwarp = (g.Y + MOMR_ROWS - 1) / MOMR_ROWS;
+        const size_t NX = 2 * P + 1;
+        const size_t tile_words = (size_t)(g.X > 32 ? 64 : 32) * 33, part_words = NX * NX * 32;
+        const size_t rsmem = (size_t)nwarp * (tile_words > part_words ? tile_words : part_words) * sizeof(float);
+#define TM_MOMR_GO(PR, PP, XH_, MAXT_, MINB_)                                                                                   \
+    do {                                                                                                                        \
+        TM_CUDA_CHECK(cudaFuncSetAttribute(loop_mom_row_kernel<PR, PP, XH_, MAXT_, MINB_>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rsmem)); \
+        loop_mom_row_kernel<PR, PP, XH_, MAXT_, MINB_><<<grid, 32 * nwarp, rsmem, st>>>(g, (const char*)a_full, (const char*)b_full, pb, w, W2); \
+    } while (0)
+        // the 32^3 x 64 ensemble shape gets the unrolled x loop and CTAs of four warps; everything else the general form
+#define TM_MOMR_LAUNCH(PR, PP)                                                                                                  \
+    do {                                                                                                                        \
+        if (g.X == 32 && nwarp <= 4) TM_MOMR_GO(PR, PP, 16, 128, MomrMinb<PR>::value);                                                  \
+        else TM_MOMR_GO(PR, PP, 0, 512, 1);                                                                                     \
+    } while (0)
+#define TM_MOMR_SWITCH(PR)                                                                                                      \
+    switch (P) {                                                                                                                \
+    case 0: TM_MOMR_LAUNCH(PR, 0); break;                                                                                       \
+    case 1: TM_MOMR_LAUNCH(PR, 1); break;                                                                                       \
+    case 2: TM_MOMR_LAUNCH(PR, 2); break;                                                                                       \
+    case 3: TM_MOMR_LAUNCH(PR, 3); break;                                                                                       \
+    default: TM_MOMR_LAUNCH(PR, 4); break;                                                                                      \
+    }
+        if (prec == 4) {
+            TM_MOMR_SWITCH(4)
+        } else {
+            TM_MOMR_SWITCH(2)
+        }
+        TM_LAUNCH_CHECK("loop_mom_row_kernel");
+        static const GammaTable tbr = make_gamma_table();
+        loop_mom_final_kernel<<<dim3(g.T, nrhs, (n_momenta + 7) / 8), 128, 0, st>>>(g, P, W2, mom_dev, n_momenta, tbr, out);
+        TM_LAUNCH_CHECK("loop_mom_final_kernel");
+        return TM_OK;
+    }
 #define TM_MOM_LAUNCH(PR, PP)                                                                                                   \
     do {                                                                                                                        \
         TM_CUDA_CHECK(cudaFuncSetAttribute(loop_mom_plane_kernel<PR, PP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
