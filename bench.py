@@ -612,10 +612,9 @@ def sweep_other_configs(torch, tm, ti, hbm_peak, out):
     X, Y, Z, T = dims
     L = tm.tm_lattice_create(dims, True)
     Vh = L.V // 2
-    per_t = X * Y * Z * 4 * 18
-    U = torch.empty(T * per_t, dtype=torch.float64, device="cuda")
-    for t0 in range(0, T, 8):
-        U[t0 * per_t:(t0 + 8) * per_t].copy_(torch.from_numpy(ti.gauge(dims, t0=t0, t1=t0 + 8).view(np.float64).reshape(-1)))
+    # 19.3 GB of canonical fp64 links: made on the device by the library's restatement of the input generator (tm_gauge_synthetic)
+    U = torch.empty(T * X * Y * Z * 4 * 18, dtype=torch.float64, device="cuda")
+    tm.tm_gauge_synthetic(L, ti.GAUGE_SEED, 1.0, ti.EPS, U)
     gauges = {}
     for prec in (4, 2):
         for recon in (18, 12):

@@ -99,6 +99,15 @@ size_t tm_spinor_bytes(const tm_lattice* L, int prec, int full, int nrhs);
 int tm_gauge_pack(const tm_lattice* L, const double* U_canonical, int prec, int recon, void* packed_out,
                   double su3_tol, void* stream);
 
+/* Synthetic SU(3) gauge field made on the device (PAPER.md:250 has sources, inversions and contractions on the
+ * GPUs -- the paper READS its gauge field from an ensemble, this call exists for the synthetic stand-in of DESIGN.md section 4): link
+ * (site, mu) = Gram-Schmidt SU(3) projection of w 1 + eps G, G complex Gaussian from the counter-based splitmix64 hash of
+ * (seed, 4 site + mu, draw), the generator of tm_inputs restated.  U_canonical_out: DEVICE fp64 [V][4][3][3][re,im] (the layout
+ * tm_gauge_pack reads).  The hashes equal the host generator's bit for bit; log / cos / sin are the device's, so every real of a link
+ * agrees with the host field to 1e-13 (measured on 32^3 x 64: median 1.1e-16, 99.99 % of the links below 2e-15, worst of 8.4 M links
+ * 1.8e-14 where a normalisation amplifies the last-bit differences) and |U U^dag - 1| < 5e-14 -- not bit-identical.  Asynchronous on `stream`. */
+int tm_gauge_synthetic(const tm_lattice* L, unsigned long long seed, double w, double eps, double* U_canonical_out, void* stream);
+
 /* Temporal gauge (reading 33; not in the paper): g(x,t) = prod_{t' < t} U_t(x,t'), U'_mu(x) = g(x) U_mu(x) g(x+mu)^dag (periodic
  * wrap; the antiperiodic sign belongs to the fermions).  U_canonical: DEVICE fp64 canonical field, transformed IN PLACE; the temporal links of
  * the slices t < T-1 are written as exactly 1 (they are 1 up to rounding), slice T-1 carries the Polyakov loop.  g_out: DEVICE fp64

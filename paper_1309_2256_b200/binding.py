@@ -27,7 +27,7 @@ ABI_SYMBOLS = [
     "tm_tsm_workspace_bytes", "tm_tsm_batch_host", "tm_launch_count", "tm_kernel_timing_enable",
     "tm_kernel_timing_read", "tm_covdev", "tm_contract_field", "tm_loop_momentum_workspace_bytes", "tm_loop_momentum",
     "tm_time_dilute", "tm_loop_contract_slice", "tm_hpe_remainder", "tm_hpe_local_traces", "tm_spinor_pack_z4_bits",
-    "tm_tsm_batch_host_bits", "tm_noise_z4", "tm_gauge_fix_temporal", "tm_kernel_signature",
+    "tm_tsm_batch_host_bits", "tm_noise_z4", "tm_gauge_fix_temporal", "tm_kernel_signature", "tm_gauge_synthetic",
 ]
 
 
@@ -101,6 +101,7 @@ def load():
         "tm_kernel_timing_enable": (i, [i]),
         "tm_kernel_timing_read": (i, [P(d), P(ctypes.c_longlong), i]),
         "tm_kernel_signature": (ctypes.c_char_p, []),
+        "tm_gauge_synthetic": (i, [vp, ctypes.c_ulonglong, d, d, vp, vp]),
         "tm_covdev": (i, [vp, vp, i, i, vp, vp, i, i, vp]),
         "tm_contract_field": (i, [vp, vp, vp, i, i, vp, vp]),
         "tm_loop_momentum_workspace_bytes": (sz, [vp, i, i, i]),
@@ -352,6 +353,10 @@ def tm_spinor_pack_z4_bits(L, codes3, prec, nrhs, packed_out, stream=None):
 
 def tm_gauge_fix_temporal(L, U_canonical, g_out, stream=None):
     return _check(load().tm_gauge_fix_temporal(L.handle, _ptr(U_canonical), _ptr(g_out), _stream(stream)), "tm_gauge_fix_temporal")
+
+
+def tm_gauge_synthetic(L, seed, w, eps, U_canonical_out, stream=None):
+    return _check(load().tm_gauge_synthetic(L.handle, int(seed), float(w), float(eps), _ptr(U_canonical_out), _stream(stream)), "tm_gauge_synthetic")
 
 
 def tm_noise_z4(L, seed, seed_stride, prec, nrhs, packed_out, stream=None):

@@ -287,7 +287,17 @@ __global__ void __launch_bounds__(BLAS_THREADS) dot_finalize_kernel(const double
     if (!c.active[rhs]) return;
     double v = 0.0;
     const double* p = partial + (size_t)rhs * ngroups;
-    for (int g = threadIdx.x; g < ngroups; g += BLAS_THREADS) v += p[g];
+    // one CTA per rhs: eight independent loads in flight per thread (the sum keeps its order, so the bits do not change);
+    // with one load per dependent add this kernel cost 16 us per call, twice per iteration
+    int g = threadIdx.x;
+    for (; g + 7 * BLAS_THREADS < ngroups; g += 8 * BLAS_THREADS) {
+        double t[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) t[k] = p[g + k * BLAS_THREADS];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v += t[k];
+    }
+    for (; g < ngroups; g += BLAS_THREADS) v += p[g];
     const double tot = block_sum(v);
     if (threadIdx.x == 0) finish_scalar<FIN>(c, rhs, tot);
 }

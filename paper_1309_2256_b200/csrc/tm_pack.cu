@@ -170,6 +170,56 @@ __global__ void noise_z4_kernel(Geo g, unsigned long long seed, unsigned long lo
     store_spinor<PREC>(packed + ((size_t)rhs * 2 + parity) * parity_bytes, g.Vh, cb, v);
 }
 
+// ---- synthetic SU(3) gauge field made on the device (SURVEY.md 8(f) NEXT-4 "on-device noise/gauge generators") --------------
+// The library's own statement of the link generator of the synthetic inputs: hashes (seed, stream 1,
+// link = 4 site + mu, draw 0..17) -> nine Box-Muller pairs -> A = w 1 + eps G -> Gram-Schmidt rows 0, 1 -> row 2 = conj(row0 x row1).
+// The hashes are bit-identical to the host generator's; log / cos / sin / sqrt are the device's fp64 routines and the products
+// may be contracted into FMAs, so the links agree with the host's to rounding (tm.h states the tolerance), not bit for bit.
+__device__ __forceinline__ double dev_u01(unsigned long long h) { return ((double)(h >> 11) + 1.0) * (1.0 / 9007199254740992.0); }
+
+__global__ void __launch_bounds__(128) gauge_synth_kernel(long long nlinks, unsigned long long seed, double w, double eps, double* __restrict__ U)
+{
+    const long long link = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (link >= nlinks) return;
+    const unsigned long long s0 = dev_splitmix64(seed ^ (1ull * 0xD6E8FEB86659FD93ULL));
+    const unsigned long long s1 = dev_splitmix64(s0 ^ ((unsigned long long)link * 0xA0761D6478BD642FULL));
+    double a[3][3][2];
+    for (int k = 0; k < 9; ++k) {
+        const unsigned long long h1 = dev_splitmix64(s1 ^ ((unsigned long long)(2 * k) * 0xE7037ED1A0B428DBULL));
+        const unsigned long long h2 = dev_splitmix64(s1 ^ ((unsigned long long)(2 * k + 1) * 0xE7037ED1A0B428DBULL));
+        const double r = sqrt(-2.0 * log(dev_u01(h1)));
+        const double ph = 6.283185307179586476925286766559 * dev_u01(h2);
+        double sn, cs;
+        sincos(ph, &sn, &cs);
+        a[k / 3][k % 3][0] = eps * (r * cs) + ((k / 3 == k % 3) ? w : 0.0);
+        a[k / 3][k % 3][1] = eps * (r * sn);
+    }
+    double n = 0;
+    for (int j = 0; j < 3; ++j) n += a[0][j][0] * a[0][j][0] + a[0][j][1] * a[0][j][1];
+    n = 1.0 / sqrt(n);
+    for (int j = 0; j < 3; ++j) { a[0][j][0] *= n; a[0][j][1] *= n; }
+    double pr = 0, pi = 0; // row0^dagger . row1
+    for (int j = 0; j < 3; ++j) {
+        pr += a[0][j][0] * a[1][j][0] + a[0][j][1] * a[1][j][1];
+        pi += a[0][j][0] * a[1][j][1] - a[0][j][1] * a[1][j][0];
+    }
+    for (int j = 0; j < 3; ++j) {
+        a[1][j][0] -= pr * a[0][j][0] - pi * a[0][j][1];
+        a[1][j][1] -= pr * a[0][j][1] + pi * a[0][j][0];
+    }
+    n = 0;
+    for (int j = 0; j < 3; ++j) n += a[1][j][0] * a[1][j][0] + a[1][j][1] * a[1][j][1];
+    n = 1.0 / sqrt(n);
+    for (int j = 0; j < 3; ++j) { a[1][j][0] *= n; a[1][j][1] *= n; }
+    for (int j = 0; j < 3; ++j) {
+        const int j1 = (j + 1) % 3, j2 = (j + 2) % 3;
+        a[2][j][0] = (a[0][j1][0] * a[1][j2][0] - a[0][j1][1] * a[1][j2][1]) - (a[0][j2][0] * a[1][j1][0] - a[0][j2][1] * a[1][j1][1]);
+        a[2][j][1] = -((a[0][j1][0] * a[1][j2][1] + a[0][j1][1] * a[1][j2][0]) - (a[0][j2][0] * a[1][j1][1] + a[0][j2][1] * a[1][j1][0]));
+    }
+    double2* dst = reinterpret_cast<double2*>(U + link * 18);
+    for (int k = 0; k < 9; ++k) dst[k] = make_double2(a[k / 3][k % 3][0], a[k / 3][k % 3][1]);
+}
+
 // ---- temporal gauge (tm.h: tm_gauge_fix_temporal) -------------------------------------------------------------------------
 __device__ __forceinline__ void cmat_mul(const double* a, const double* b, double* c, bool bdag) // c = a b  or  a b^dag
 {
@@ -358,6 +408,16 @@ extern "C" int tm_spinor_pack_z4_bits(const tm_lattice* L, const unsigned char* 
     if (!L || !codes3 || !out || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
     if (!aligned256(codes3) || !aligned256(out)) return TM_ERR_LAYOUT;
     return spinor_pack_any(L->g, L->V, prec, 3, nullptr, nullptr, codes3, out, nrhs, (cudaStream_t)stream);
+}
+
+extern "C" int tm_gauge_synthetic(const tm_lattice* L, unsigned long long seed, double w, double eps, double* U_canonical_out, void* stream)
+{
+    if (!L || !U_canonical_out) return TM_ERR_ARG;
+    if (!aligned256(U_canonical_out)) return TM_ERR_LAYOUT;
+    const long long nlinks = L->V * 4;
+    gauge_synth_kernel<<<(unsigned)((nlinks + 127) / 128), 128, 0, (cudaStream_t)stream>>>(nlinks, seed, w, eps, U_canonical_out);
+    TM_LAUNCH_CHECK("gauge_synth_kernel");
+    return TM_OK;
 }
 
 extern "C" int tm_noise_z4(const tm_lattice* L, unsigned long long seed, unsigned long long seed_stride, int prec, int nrhs,

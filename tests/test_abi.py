@@ -82,6 +82,7 @@ def test_every_wrapper_reaches_the_library(tm):
         lambda: tm.tm_spinor_pack_z4(L, None, 4, 1, buf, stream=0),
         lambda: tm.tm_spinor_pack_z4_bits(L, None, 4, 1, buf, stream=0),
         lambda: tm.tm_noise_z4(L, 1, 1, 4, 1, None, stream=0),
+        lambda: tm.tm_gauge_synthetic(L, 1, 1.0, 0.5, None, stream=0),
         lambda: tm.tm_dslash(L, None, 4, 18, buf, buf, None, 0, 0, 0, 0.1, 0.0, 1, stream=0),
         lambda: tm.tm_dslash_general(L, None, 4, 18, buf, buf, None, 0, 0, (0, 0, 1, 0), 1, stream=0),
         lambda: tm.tm_MdagM(L, None, 4, 18, buf, buf, buf, 0, 0.1, 0.0, 1, stream=0),
