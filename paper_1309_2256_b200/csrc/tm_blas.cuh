@@ -38,9 +38,10 @@ struct BlasCtx {
 enum { FIN_AUX = 0, FIN_PAP = 1, FIN_RR = 2, FIN_INIT = 3 };
 
 // block-wide sum of `v` (all threads call); result valid in thread 0
+template <int THREADS = BLAS_THREADS>
 __device__ __forceinline__ double block_sum(double v)
 {
-    __shared__ double sm[BLAS_THREADS / 32];
+    __shared__ double sm[THREADS / 32];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -49,7 +50,7 @@ __device__ __forceinline__ double block_sum(double v)
     __syncthreads();
     double s = 0.0;
     if (threadIdx.x < 32) {
-        s = (threadIdx.x < BLAS_THREADS / 32) ? sm[threadIdx.x] : 0.0;
+        s = (threadIdx.x < THREADS / 32) ? sm[threadIdx.x] : 0.0;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
     }
@@ -280,25 +281,25 @@ __global__ void __launch_bounds__(BLAS_THREADS) axpby_kernel(int Vh, VecArg y_, 
 //   partials in a fixed order -> alpha / beta, convergence;  update_xp: x += alpha p, p = r + beta p (5 vector passes).
 
 // tot[rhs] = sum_g partial[rhs][g] (fixed order), then the FIN scalar update (FIN_PAP or FIN_RR).  grid = nrhs blocks
+constexpr int FIN_THREADS = 1024; // one CTA per rhs sums 32 768 partials at 32^3 x 64: latency-bound, so many threads and loads in flight
 template <int FIN>
-__global__ void __launch_bounds__(BLAS_THREADS) dot_finalize_kernel(const double* partial, int ngroups, BlasCtx c)
+__global__ void __launch_bounds__(FIN_THREADS) dot_finalize_kernel(const double* partial, int ngroups, BlasCtx c)
 {
     const int rhs = blockIdx.x;
     if (!c.active[rhs]) return;
     double v = 0.0;
     const double* p = partial + (size_t)rhs * ngroups;
-    // one CTA per rhs: eight independent loads in flight per thread (the sum keeps its order, so the bits do not change);
-    // with one load per dependent add this kernel cost 16 us per call, twice per iteration
+    // fixed order: thread k sums partials k, k + FIN_THREADS, ... (eight independent loads in flight), then the block tree
     int g = threadIdx.x;
-    for (; g + 7 * BLAS_THREADS < ngroups; g += 8 * BLAS_THREADS) {
+    for (; g + 7 * FIN_THREADS < ngroups; g += 8 * FIN_THREADS) {
         double t[8];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) t[k] = p[g + k * BLAS_THREADS];
+        for (int k = 0; k < 8; ++k) t[k] = p[g + k * FIN_THREADS];
 #pragma unroll
         for (int k = 0; k < 8; ++k) v += t[k];
     }
-    for (; g < ngroups; g += BLAS_THREADS) v += p[g];
-    const double tot = block_sum(v);
+    for (; g < ngroups; g += FIN_THREADS) v += p[g];
+    const double tot = block_sum<FIN_THREADS>(v);
     if (threadIdx.x == 0) finish_scalar<FIN>(c, rhs, tot);
 }
 

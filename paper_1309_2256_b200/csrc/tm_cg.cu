@@ -115,7 +115,7 @@ static int k_cg_iter_fused(const Geo& g, const void* gauge, int prec, int recon,
     d.dot_partial = partial;
     if ((rc = launch_dslash(g, prec, recon, d, st)) != TM_OK) return rc;
     d.dot_partial = nullptr;
-    dot_finalize_kernel<FIN_PAP><<<nrhs, BLAS_THREADS, 0, st>>>(partial, ngroups, c);
+    dot_finalize_kernel<FIN_PAP><<<nrhs, FIN_THREADS, 0, st>>>(partial, ngroups, c);
     TM_LAUNCH_CHECK("dot_finalize_kernel");
     d.out = t1; d.in = t2; d.x = nullptr; d.out_parity = 1; d.dagger = 1; d.rhs_stride_x = pb;
     kind_pq(TM_KIND_TWIST_INV, 1, kappa, mu, d.pq);
@@ -126,7 +126,7 @@ static int k_cg_iter_fused(const Geo& g, const void* gauge, int prec, int recon,
     d.axpy_coef = &c.scal[0].alpha; d.axpy_coef_stride = sizeof(CgScal);
     d.dot_partial = partial;
     if ((rc = launch_dslash(g, prec, recon, d, st)) != TM_OK) return rc;
-    dot_finalize_kernel<FIN_RR><<<nrhs, BLAS_THREADS, 0, st>>>(partial, ngroups, c);
+    dot_finalize_kernel<FIN_RR><<<nrhs, FIN_THREADS, 0, st>>>(partial, ngroups, c);
     TM_LAUNCH_CHECK("dot_finalize_kernel");
     dim3 grid(blas_blocks(g.Vh), nrhs);
     return by_prec(prec, [&](auto P) {
