@@ -544,6 +544,22 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world):
                                                  "true_resid_full_system": max(x.true_resid for x in info), "seconds": dt,
                                                  "ms_per_solve": 1e3 * dt / NRHS, "HP_solves_per_s": NRHS / dt}
         del ws
+    # ... and ONE source through the same mode (configs[2]'s "mixed-precision CG to 1e-8 on one Z2xiZ2 source"): nrhs = 1 takes the
+    # fused single-rhs iteration without a link cache
+    for plp in (4, 2):
+        ws = tm.device_buffer(tm.tm_cg_workspace_bytes(L, 8, plp, tm.TM_CG_HP_DEFECT, 1))
+        prm = tm.make_cg_params(kappa, mu, 1e-8, 5000, tm.TM_CG_HP_DEFECT, 0.0)
+        best = None
+        for rep in range(2):
+            torch.cuda.synchronize()
+            t0 = time.time()
+            rc, info = tm.tm_cg_multi(L, gauges[(8, 12)], 8, gauges[(plp, 12)], plp, 12, sN[:pb8], etaN[:pb8], prm, 1, ws)
+            torch.cuda.synchronize()
+            dt = time.time() - t0
+            best = dt if best is None else min(best, dt)
+        cg["defect_x1_fp64+fp%d" % (plp * 8)] = {"status": rc, "inner_iters": info[0].iters, "cycles": info[0].reliable_updates,
+                                                "true_resid_full_system": info[0].true_resid, "seconds": best}
+        del ws
     del etaN, sN, c1
     out["cg_mixed_1e-8"] = cg
     # the paper's per-configuration TSM workload (N_HP = 8, N_LP = 200) from the rates measured above

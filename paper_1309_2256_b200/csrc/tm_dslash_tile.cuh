@@ -453,7 +453,11 @@ __device__ __forceinline__ void tile_site2(const DslashKArgs& a, const SM& sm, i
             const char* blk = a.gauge + (size_t)((fwd ? a.parity : 1 - a.parity) * 4 + (d >> 1)) * a.link_block;
             // temporal gauge declared (RECON = reals + 200): a temporal hop that does not wrap around crosses a unit link
             const bool unit_hop = RECON >= 200 && ((d == 6 && nb[6] > cb) || (d == 7 && nb[7] < cb));
+#ifdef TM_DEBUG_LINKWIN // timing ablation (probe builds only, wrong results): every link load lands in a 1024-site window (L1 / L2 hits)
+            if (!unit_hop) load_link<PREC, RECON>(blk, Vh, (fwd ? cb : nb[d]) & 1023, u);
+#else
             if (!unit_hop) load_link<PREC, RECON>(blk, Vh, fwd ? cb : nb[d], u);
+#endif
         }
         float h[12];
         float w = 1.f;

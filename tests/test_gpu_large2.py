@@ -139,6 +139,25 @@ def test_32x64_hp_defect_twelve_sources():
         assert res <= 1.05 * tol and abs(res - info[r].true_resid) <= 0.05 * tol
 
 
+def test_32x64_hp_defect_one_source():
+    """bench.py `cg_mixed_1e-8.defect_x1_fp64+fp16` (configs[2]: mixed-precision CG to 1e-8 on ONE source): nrhs = 1 runs the fused
+    single-rhs iteration without a link cache; full-system residual recomputed with the oracle's operator."""
+    tol = 1e-8
+    U = ti.gauge(DIMS)
+    F = Fields(DIMS, U, True)
+    e = ti.z4(DIMS, seed=ti.NOISE_SEED + 77)
+    eta = F.pack(e, 8)
+    g8, g2 = F.gauge(8, 12), F.gauge(2, 12)
+    F.drop_canonical()
+    s = F.zeros_full(8)
+    ws = tm.device_buffer(tm.tm_cg_workspace_bytes(F.L, 8, 2, tm.TM_CG_HP_DEFECT, 1))
+    prm = tm.make_cg_params(KAPPA, MU, tol, 5000, tm.TM_CG_HP_DEFECT, 0.0)
+    rc, info = tm.tm_cg_multi(F.L, g8, 8, g2, 2, 12, s, eta, prm, 1, ws)
+    assert rc == tm.TM_OK and info[0].status == tm.TM_OK and 0 < info[0].true_resid <= tol
+    res = np.linalg.norm((e - oracle.M(U, F.unpack(s, 8), KAPPA, MU)).ravel()) / np.linalg.norm(e.ravel())
+    assert res <= 1.05 * tol and abs(res - info[0].true_resid) <= 0.05 * tol
+
+
 def test_64x128_xpay_twist_sampled_sites():
     """configs[4] `xpay_twist_*` rows: out = R(+-a) x - kappa^2 D in (dagger too), fp32 and fp16 storage, 18- and 12-real links,
     on ~3e4 sampled sites per case (random + two planes that touch every wrap-around) against the single-site oracle."""
