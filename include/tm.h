@@ -67,7 +67,7 @@ typedef enum {
     TM_ERR_CUDA = -4,      /* CUDA runtime error (no device, launch failure); tm_last_cuda_error() has the text */
     TM_ERR_BREAKDOWN = -5, /* CG: <p,Ap> <= 0 or NaN */
     TM_ERR_MAXITER = -6,   /* CG: max_iter reached before tol (solution still returned) */
-    TM_ERR_RECON8 = -7,    /* tm_gauge_pack with recon 8: a link has |U01|^2 + |U02|^2 < 1e-6, where the 8-real chart is singular */
+    TM_ERR_RECON8 = -7,    /* tm_gauge_pack with recon 8: a link has |U00|^2 + |U01|^2 < 1e-6 (|U02| = 1), where the 8-real chart is singular */
     TM_ERR_NOT_TGAUGE = -8 /* tm_gauge_pack with a *_TG code: a temporal link of a slice t < T-1 is not exactly the unit matrix */
 } tm_status;
 
@@ -92,10 +92,12 @@ size_t tm_spinor_bytes(const tm_lattice* L, int prec, int full, int nrhs);
  * recon 12 keeps rows 0,1 (row 2 = conj(row0 x row1) is rebuilt in the kernels; the antiperiodic sign is NOT
  * folded into stored links).  With recon 12, returns TM_ERR_NOT_SU3 if max |U U^dag - 1|, |row2 - conj(r0 x r1)|
  * exceeds su3_tol (this check synchronises the stream); su3_tol <= 0 skips the check.
- * recon 8 ("8-parameter reconstruction"): U01, U02, U10 and arg(U00)/pi, arg(U20)/pi are stored; the kernels rebuild
- * the link from unitarity (two square roots, two sincospi, one reciprocal of r = |U01|^2 + |U02|^2: errors grow like 1/r, so
- * links with U00 of modulus ~1 lose accuracy; reading 31).  Same SU(3) check as recon 12; a field with a link of
- * r < 1e-6 (the unit link has r = 0) is refused with TM_ERR_RECON8 (this check always synchronises the stream). */
+ * recon 8 ("8-parameter reconstruction"): of V = U P, V_ij = U_{i,(j+2)%3} (columns shifted cyclically; still SU(3)) the
+ * numbers V01, V02, V10 and arg(V00)/pi, arg(V20)/pi are stored; the kernels rebuild V from unitarity (two square roots, two sincospi,
+ * one reciprocal of r = |V01|^2 + |V02|^2 = |U00|^2 + |U01|^2: errors grow like 1/r; reading 31) and undo the shift by
+ * renaming.  The shift puts the chart's singular set at |U02| = 1 instead of the unit link, so free fields and temporal-gauge
+ * fields pack.  Same SU(3) check as recon 12; a field with a link of r < 1e-6 is refused with TM_ERR_RECON8 (this check always
+ * synchronises the stream). */
 int tm_gauge_pack(const tm_lattice* L, const double* U_canonical, int prec, int recon, void* packed_out,
                   double su3_tol, void* stream);
 

@@ -210,7 +210,9 @@ __device__ __forceinline__ void rebuild_row2(real* u)
     }
 }
 
-// 8 stored reals q = (U01, U02, U10, arg U00 / pi, arg U20 / pi) -> u[18].  Unitarity of row 0 and column 0 gives |U00|, |U20|;
+// 8 stored reals q = (V01, V02, V10, arg V00 / pi, arg V20 / pi) of V = U P, V_ij = U_{i,(j+2)%3} (a cyclic column shift: det P = 1, so V
+// is in SU(3); it moves the chart's singular set V01 = V02 = 0 from the unit link -- which every free field and every temporal-gauge
+// field is full of -- to |U02| = 1) -> u[18].  Unitarity of row 0 and column 0 gives |U00|, |U20|;
 // row 1 follows from  row1 . conj(row0) = 0  and  (row0 x row1)_0 = conj(U20)  (two linear equations in U11, U12 with determinant
 // r = |U01|^2 + |U02|^2), row 2 = conj(row0 x row1).  Ill-conditioned as r -> 0 (errors grow like 1/r).
 template <typename real>
@@ -234,9 +236,18 @@ __device__ __forceinline__ void rebuild_from8(const real* q, real* u)
     // U12 = (conj(U01 U20) - t U02) / r
     const real wr = a1r * u20r - a1i * u20i, wi = a1r * u20i + a1i * u20r; // U01 U20
     const real u12r = (wr - (tr * a2r - ti * a2i)) * rinv, u12i = (-wi - (tr * a2i + ti * a2r)) * rinv;
-    u[0] = u00r; u[1] = u00i; u[2] = a1r; u[3] = a1i; u[4] = a2r; u[5] = a2i;
-    u[6] = br; u[7] = bi; u[8] = u11r; u[9] = u11i; u[10] = u12r; u[11] = u12i;
-    rebuild_row2(u);
+    real v[18]; // the stored matrix is V = U P (columns shifted cyclically, below)
+    v[0] = u00r; v[1] = u00i; v[2] = a1r; v[3] = a1i; v[4] = a2r; v[5] = a2i;
+    v[6] = br; v[7] = bi; v[8] = u11r; v[9] = u11i; v[10] = u12r; v[11] = u12i;
+    rebuild_row2(v);
+    // U_{i,(j+2)%3} = V_{ij}: undoing the column shift is a renaming of registers
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            u[2 * (i * 3 + (j + 2) % 3)] = v[2 * (i * 3 + j)];
+            u[2 * (i * 3 + (j + 2) % 3) + 1] = v[2 * (i * 3 + j) + 1];
+        }
 }
 
 template <int PREC, int RECON_CODE>

@@ -76,10 +76,16 @@ __global__ void gauge_pack_kernel(Geo g, const double* __restrict__ U, char* out
         if (!(dev == dev)) dev = 1e30; // NaN
         atomicMax(&g_su3_dev_bits, __float_as_uint((float)dev));
     }
-    if (RECON == 8) { // U01, U02, U10, arg(U00)/pi, arg(U20)/pi (tm_layout.cuh rebuild_from8)
-        const double r8 = u[2] * u[2] + u[3] * u[3] + u[4] * u[4] + u[5] * u[5];
+    if (RECON == 8) { // V01, V02, V10, arg(V00)/pi, arg(V20)/pi of V_ij = U_{i,(j+2)%3} (tm_layout.cuh rebuild_from8)
+        double v[18];
+        for (int i = 0; i < 3; ++i)
+            for (int j = 0; j < 3; ++j) {
+                v[2 * (i * 3 + j)] = u[2 * (i * 3 + (j + 2) % 3)];
+                v[2 * (i * 3 + j) + 1] = u[2 * (i * 3 + (j + 2) % 3) + 1];
+            }
+        const double r8 = v[2] * v[2] + v[3] * v[3] + v[4] * v[4] + v[5] * v[5];
         atomicMax(&g_r8_inv_bits, __float_as_uint(r8 > 1e-30 ? (float)fmin(1.0 / r8, 1e30) : 1e30f));
-        double q[8] = {u[2], u[3], u[4], u[5], u[6], u[7], atan2(u[1], u[0]) / 3.14159265358979323846, atan2(u[13], u[12]) / 3.14159265358979323846};
+        double q[8] = {v[2], v[3], v[4], v[5], v[6], v[7], atan2(v[1], v[0]) / 3.14159265358979323846, atan2(v[13], v[12]) / 3.14159265358979323846};
         store_reals<PREC>(out + (size_t)pm * link_block, g.Vh, cb, q, 8);
         return;
     }

@@ -139,12 +139,16 @@ def test_dslash_all_kinds(dims, prec, recon):
 
 
 def test_gauge_pack_recon8_refuses_the_singular_chart():
-    """The unit link has U01 = U02 = 0: the 8 stored reals do not determine it (reading 31)."""
+    """The stored matrix is V = U P (columns shifted cyclically, reading 31): the chart is singular where V01 = V02 = 0,
+    i.e. |U02| = 1 -- not at the unit link, which packs (free fields, temporal-gauge fields)."""
     dims = (4, 4, 4, 4)
     L = tm.tm_lattice_create(dims)
     buf = tm.device_buffer(tm.tm_gauge_bytes(L, 4, 8))
+    tm.tm_gauge_pack(L, to_dev(ti.unit_gauge(dims)), 4, 8, buf, 1e-10)
+    bad = ti.unit_gauge(dims).copy()
+    bad[2, 1, 0, 3, 1] = np.array([[0, 0, 1], [1, 0, 0], [0, 1, 0]], dtype=np.complex128)  # an SU(3) link with |U02| = 1
     with pytest.raises(tm.TmError) as e:
-        tm.tm_gauge_pack(L, to_dev(ti.unit_gauge(dims)), 4, 8, buf, 1e-10)
+        tm.tm_gauge_pack(L, to_dev(bad), 4, 8, buf, 1e-10)
     assert e.value.status == tm.TM_ERR_RECON8
     U = ti.gauge(dims).copy()
     U[1, 2, 3, 0, 2, 1, 1] *= 1.01
@@ -155,9 +159,10 @@ def test_gauge_pack_recon8_refuses_the_singular_chart():
     assert tm.tm_gauge_bytes(L, 4, 8) * 18 == tm.tm_gauge_bytes(L, 4, 18) * 8
 
 
-@pytest.mark.parametrize("prec,recon", [(8, 18), (8, 12), (4, 12), (2, 12), (2, 18)])
+@pytest.mark.parametrize("prec,recon", [(8, 18), (8, 12), (4, 12), (2, 12), (2, 18), (8, 8), (4, 8), (2, 8)])
 def test_dslash_free_field_plane_wave(prec, recon):
-    """P2 through the GPU: U = 1, odd temporal momentum across the antiperiodic boundary, both reconstructs."""
+    """P2 through the GPU: U = 1, odd temporal momentum across the antiperiodic boundary, all three reconstructs (the unit link is a
+    regular point of the 8-real chart since the stored matrix is U P)."""
     dims = (4, 6, 4, 8)
     F, U = fields(dims, unit=True)
     X, Y, Z, T = dims
