@@ -8,7 +8,7 @@ storage / fp32 arithmetic / fp64 reductions, 12-real links, every gauge load sha
 The same run also reports BASELINE.json's other metric, single-RHS tm-dslash GFLOPS and algorithmic HBM GB/s at
 fp32 / fp16 x 18 / 12 reals (configs[2]), and a mixed-precision CG to 1e-8.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--no-sweeps]
 N > 1: launched under torch.distributed.run; noise sources are independent, so ranks take different batches and
 there is no data-path collective (weak scaling, "replicas + gather" of the [16][T] loops through paper_1309_2256_b200.shard).
 """
@@ -292,7 +292,7 @@ def run_b200(args, rank, world, local_rank):
         out["dslash"] = table
         out["dslash_peak_source"] = peak_src
         extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world, table)
-        if args.sweeps and world == 1:
+        if not args.no_sweeps and world == 1:
             del gauges, eta, sol, cg_ws, tsm_ws
             torch.cuda.empty_cache()
             sweep_other_configs(torch, tm, ti, hbm_peak, out)
@@ -682,6 +682,11 @@ def sweep_other_configs(torch, tm, ti, hbm_peak, out):
                     "us": ms * 1e3, "GFLOPS": Vh * fl / ms / 1e6, "GBps_algorithmic": by / ms / 1e6,
                     "frac_of_measured_%.0f" % hbm_peak: by / ms / 1e6 / hbm_peak, "frac_of_nominal_8000": by / ms / 1e6 / 8000.0}
         del src, o, x, tmp
+    for prec_, nm in ((4, "fp32"), (2, "fp16")):  # flat scalars where the driver's parse keeps them (TWIST_INV, single rhs, 64^3x128)
+        for rc_ in (18, 12):
+            row = big["twist_inv_fp%d_recon%d" % (prec_ * 8, rc_)]
+            out["roofline"]["dslash64_%s_r%d_frac" % (nm, rc_)] = row["frac_of_measured_%.0f" % hbm_peak]
+            out["roofline"]["dslash64_%s_r%d_us" % (nm, rc_)] = row["us"]
     out["config4_64x128"] = {"note": "33.5 M sites; gauge 3.2-9.7 GB + spinors 0.9-1.6 GB per parity: every launch streams from HBM",
                              "table": big}
 
@@ -729,7 +734,8 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--sweeps", action="store_true", help="also time BASELINE.json configs[1] (16^3x32, CUDA graph) and [4] (64^3x128)")
+    ap.add_argument("--sweeps", action="store_true", help="kept for compatibility: configs[1] and [4] are timed by default now")
+    ap.add_argument("--no-sweeps", action="store_true", help="skip BASELINE.json configs[1] (16^3x32, CUDA graph) and [4] (64^3x128; needs ~35 GB of HBM, ~6 s)")
     ap.add_argument("--dry-run", action="store_true", help="CPU / gloo run of the launcher and the multi-rank host logic only (no GPU, no timing)")
     args = ap.parse_args()
     if args.gpus < 1:
