@@ -48,6 +48,19 @@ def ncu_traffic(signature):
     return float(rec["dram_bytes_per_launch"]), "%s: %s" % (os.path.relpath(TRAFFIC_RECORD, ROOT), rec.get("source", ""))
 
 
+def ncu_pipe_fractions(signature):
+    """FMA-pipe and issue-slot utilisation of the dominant kernel from the same signature-checked ncu record ({} when stale):
+    the counted flops (1392 / 1416 per site) leave out conversion, projection, link handling and epilogue work, so `frac`
+    understates how busy the FP32 pipe is."""
+    try:
+        rec = json.load(open(TRAFFIC_RECORD))
+    except Exception:
+        return {}
+    if rec.get("signature") != signature:
+        return {}
+    return {k + "_ncu": rec[k] for k in ("fma_pipe_active_frac", "issue_active_frac") if k in rec}
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -277,6 +290,7 @@ def run_b200(args, rank, world, local_rank):
                 "avg_launch_ms": k_avg_ms, "launches_timed": int(k_n), "share_of_step": k_ms / (ms_step * args.steps),
                 # the same launches in the HBM view (flat scalars: nested objects do not survive the driver's parse)
                 "hbm_achieved_GBps": ach_gbs, "hbm_peak_GBps": hbm_peak, "hbm_frac": ach_gbs / hbm_peak, "hbm_peak_source": peak_src}
+    roofline.update(ncu_pipe_fractions(sig))
 
     out = {"metric": "LP solves/s", "value": value, "unit": "solves/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
