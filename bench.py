@@ -604,6 +604,49 @@ def extras(torch, tm, ti, L, gauges, hbm_peak, peak_src, out, world, table):
             "note": "derived: N_HP solves to 1e-8 (batched defect correction) + (N_HP + N_LP) truncated solves with their loops, at the "
                     "rates measured in this run on the synthetic eps = 0.5 field (9 / 62 iterations; a physical light-quark ensemble "
                     "needs about 10x more).  Context: PAPER.md Table I R_HP/LP = 17-27 (light, strange), Table II 1471 GPU-node-seconds"}
+    # ... and the same workload actually RUN: all sources made on the device (tm_noise_z4), N_HP = 8 sources solved to 1e-8 (batched defect
+    # correction, fp64 loops), the same 8 and 200 further sources solved in the truncated mode in batches of 12, every solution contracted
+    # (16 Gamma x T), Eq. (8) combined on the device (tm_tsm_combine).  Wall clock around the whole configuration, one stream.
+    n_hp, n_lp, T = 8, 200, DIMS[3]
+    seed0 = ti.NOISE_SEED + 5000
+    fb2_ = tm.tm_spinor_bytes(L, 2, 1, NRHS)
+    e2_, s2_ = tm.device_buffer(fb2_), tm.device_buffer(fb2_)
+    fb8_ = tm.tm_spinor_bytes(L, 8, 1, n_hp)
+    e8_, s8_ = tm.device_buffer(fb8_), tm.device_buffer(fb8_)
+    ws_lp = tm.device_buffer(tm.tm_cg_workspace_bytes(L, 8, 2, tm.TM_CG_LP_TRUNCATED, NRHS))
+    ws_hp = tm.device_buffer(tm.tm_cg_workspace_bytes(L, 8, 2, tm.TM_CG_HP_DEFECT, n_hp))
+    lws_ = tm.device_buffer(tm.tm_loop_workspace_bytes(L, NRHS))
+    l_hp = torch.zeros((n_hp, 16, T, 2), dtype=torch.float64, device="cuda")
+    l_lp = torch.zeros((n_hp + n_lp, 16, T, 2), dtype=torch.float64, device="cuda")
+    l_out = torch.zeros((16, T, 2), dtype=torch.float64, device="cuda")
+    prm_lp = tm.make_cg_params(kappa, mu, LP_TOL, 500, tm.TM_CG_LP_TRUNCATED, 0.1, 0, 1)
+    prm_hp = tm.make_cg_params(kappa, mu, 1e-8, 5000, tm.TM_CG_HP_DEFECT, 0.0)
+
+    def configuration():
+        tm.tm_noise_z4(L, seed0, 1, 8, n_hp, e8_)
+        rc, _ = tm.tm_cg_multi(L, gauges[(8, 12)], 8, gauges[(2, 12)], 2, 12, s8_, e8_, prm_hp, n_hp, ws_hp)
+        assert rc == tm.TM_OK, rc
+        tm.tm_loop_contract(L, e8_, s8_, 8, n_hp, l_hp, lws_)
+        for first in range(0, n_hp + n_lp, NRHS):
+            n = min(NRHS, n_hp + n_lp - first)
+            tm.tm_noise_z4(L, seed0 + first, 1, 2, n, e2_)
+            rc, _ = tm.tm_cg_multi(L, None, 8, gauges[(2, 12)], 2, 12, s2_, e2_, prm_lp, n, ws_lp)
+            assert rc == tm.TM_OK, rc
+            tm.tm_loop_contract(L, e2_, s2_, 2, n, l_lp[first:first + n], lws_)
+        tm.tm_tsm_combine(T, l_hp, l_lp[:n_hp], n_hp, l_lp[n_hp:], n_lp, l_out)
+
+    configuration()
+    torch.cuda.synchronize()
+    t0 = time.time()
+    configuration()
+    torch.cuda.synchronize()
+    dt_cfg = time.time() - t0
+    tr = l_out.cpu().numpy()
+    out["tsm_configuration_measured"] = {"n_hp": n_hp, "n_lp": n_lp, "seconds": dt_cfg, "solves": 2 * n_hp + n_lp,
+                                         "loop_Gamma0_t0_re": float(tr[0, 0, 0]), "loop_Gamma15_t0_im": float(tr[15, 0, 1]),
+                                         "note": "one configuration of the paper's TSM workload (PAPER.md:106, :226) run end to end on the device: noise, "
+                                                 "8 HP + 208 LP solves, 216 contractions, Eq. (8); synthetic field (9 / 63 iterations per solve)"}
+    del e2_, s2_, e8_, s8_, ws_lp, ws_hp, lws_
     if world == 1:
         # ~26 s of oracle work on the GPU box; the --impl reference arm keeps the 1.5 s sample so that its K + W steps stay short
         base, _ = cpu_oracle_sample(large=True)
