@@ -235,6 +235,35 @@ def test_cg_lp_truncated_ragged_6x6x6x6():
     assert torch.equal(s1, s[5 * fb:6 * fb])
 
 
+@pytest.mark.parametrize("nrhs", [7, 8, 9])
+@pytest.mark.parametrize("prec", [2, 4])
+def test_cg_lp_truncated_seven_to_nine_rhs(nrhs, prec):
+    """7 and 8 right-hand sides take the 8-rhs launch shape of the link-cache kernel (the last batch of 200 sources, N_HP = 8), 9 the
+    12-rhs shape with three idle rows: oracle iteration counts, and every source bit-equal to its unbatched solve."""
+    dims = (6, 6, 6, 6)
+    F, U = fields(dims)
+    recon = 12
+    eta = np.stack([ti.z4(dims, seed=820 + r) for r in range(nrhs)])
+    pe = F.pack(eta, prec)
+    s = F.zeros_full(prec, nrhs)
+    ws = tm.device_buffer(tm.tm_cg_workspace_bytes(F.L, 8, prec, tm.TM_CG_LP_TRUNCATED, nrhs))
+    prm = tm.make_cg_params(KAPPA, MU, 1e-2, 500, tm.TM_CG_LP_TRUNCATED)
+    rc, info = tm.tm_cg_multi(F.L, None, 8, F.gauge(prec, recon), prec, recon, s, pe, prm, nrhs, ws)
+    assert rc == tm.TM_OK
+    got = F.unpack(s, prec, nrhs=nrhs)
+    s_ref, iref = oracle.cg_solve(U, eta[nrhs - 1], KAPPA, MU, 1e-2, 500)
+    assert abs(info[nrhs - 1].iters - iref["iters"]) <= 2 and rel(got[nrhs - 1], s_ref) < 3e-2
+    fb = tm.tm_spinor_bytes(F.L, prec, 1, 1)
+    ws1 = tm.device_buffer(tm.tm_cg_workspace_bytes(F.L, 8, prec, tm.TM_CG_LP_TRUNCATED, 1))
+    e1, s1 = tm.device_buffer(fb), tm.device_buffer(fb)
+    for r in (0, nrhs - 1):
+        e1.copy_(pe[r * fb:(r + 1) * fb])
+        s1.zero_()
+        rc1, info1 = tm.tm_cg(F.L, None, 8, F.gauge(prec, recon), prec, recon, s1, e1, prm, ws1)
+        assert rc1 == tm.TM_OK and info1.iters == info[r].iters
+        assert torch.equal(s1, s[r * fb:(r + 1) * fb])
+
+
 def test_cg_breakdown_is_per_rhs():
     """A NaN source makes <p,Ap> NaN: that right-hand side stops with TM_ERR_BREAKDOWN, the others of the batch converge."""
     dims = (4, 4, 4, 8)
