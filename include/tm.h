@@ -68,7 +68,8 @@ typedef enum {
     TM_ERR_BREAKDOWN = -5, /* CG: <p,Ap> <= 0 or NaN */
     TM_ERR_MAXITER = -6,   /* CG: max_iter reached before tol (solution still returned) */
     TM_ERR_RECON8 = -7,    /* tm_gauge_pack with recon 8: a link has |U00|^2 + |U01|^2 < 1e-6 (|U02| = 1), where the 8-real chart is singular */
-    TM_ERR_NOT_TGAUGE = -8 /* tm_gauge_pack with a *_TG code: a temporal link of a slice t < T-1 is not exactly the unit matrix */
+    TM_ERR_NOT_TGAUGE = -8, /* tm_gauge_pack with a *_TG code: a temporal link of a slice t < T-1 is not exactly the unit matrix */
+    TM_ERR_STATIC_LIMIT = -9 /* tm_loop_contract_static: the call needs more than TM_LOOP_STATIC_BYTES of scratch; use tm_loop_contract */
 } tm_status;
 
 #define TM_MAX_NRHS 16
@@ -204,6 +205,21 @@ int tm_cg(const tm_lattice* L, const void* gauge_hp, int prec_hp, const void* ga
 size_t tm_loop_workspace_bytes(const tm_lattice* L, int nrhs);
 int tm_loop_contract(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, double* out,
                      void* workspace, void* stream);
+
+/* The same contraction for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): no workspace argument -- the per-block partial sums live in a file-scope device array of
+ * TM_LOOP_STATIC_BYTES (8 MiB) that every GPU which loads the library holds until the process exits.  Inputs, output, arithmetic
+ * and results are those of tm_loop_contract (same kernels, bit-equal).  The call performs no cudaMalloc / cudaFree and calls no
+ * allocating library routine.  Limit: tm_loop_workspace_bytes(L, nrhs) <= TM_LOOP_STATIC_BYTES, i.e. nrhs * T * nb <= 32768 with
+ * nb = min(32, max(1, X*Y*Z/2048)) -- 32^3 x 64 up to 16 right-hand sides per call, 64^3 x 128 up to 8; beyond it the call returns
+ * TM_ERR_STATIC_LIMIT and launches nothing.  The first call on a device looks the array's device address up
+ * (cudaGetSymbolAddress, once per device, with that device current): make that first call outside stream capture.
+ * ALL calls of a process share the one array per device, which keeps the contents of the last call (nothing in it has to start at
+ * zero: every partial is written before it is read): two calls that overlap on one GPU (different streams, or different host
+ * threads) RACE on it -- keep calls on one stream, or order them with events. */
+#define TM_LOOP_STATIC_BYTES 8388608
+int tm_loop_contract_static(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, double* out,
+                            void* stream);
 
 /* ---- NEXT-1: estimators built from the rows above ------------------------------------------ */
 /* a8': out[rhs][n][t] = scale * sum_{x: x4=t} (g5^g5_left a)^dag (Gamma_n x 1) (g5^g5_right b), scale = scale_re + i scale_im.

@@ -17,6 +17,8 @@ TM_CG_HP_MIXED, TM_CG_LP_TRUNCATED, TM_CG_HP_DEFECT = 0, 1, 2
 TM_ONEEND_TAU3, TM_ONEEND_GENERAL = 0, 1
 TM_OK, TM_ERR_ARG, TM_ERR_LAYOUT, TM_ERR_NOT_SU3, TM_ERR_CUDA, TM_ERR_BREAKDOWN, TM_ERR_MAXITER, TM_ERR_RECON8 = 0, -1, -2, -3, -4, -5, -6, -7
 TM_ERR_NOT_TGAUGE = -8
+TM_ERR_STATIC_LIMIT = -9
+TM_LOOP_STATIC_BYTES = 8388608
 TM_MAX_NRHS = 16
 
 ABI_SYMBOLS = [
@@ -27,7 +29,7 @@ ABI_SYMBOLS = [
     "tm_tsm_workspace_bytes", "tm_tsm_batch_host", "tm_launch_count", "tm_kernel_timing_enable",
     "tm_kernel_timing_read", "tm_covdev", "tm_contract_field", "tm_loop_momentum_workspace_bytes", "tm_loop_momentum",
     "tm_time_dilute", "tm_loop_contract_slice", "tm_hpe_remainder", "tm_hpe_local_traces", "tm_spinor_pack_z4_bits",
-    "tm_tsm_batch_host_bits", "tm_noise_z4", "tm_gauge_fix_temporal", "tm_kernel_signature", "tm_gauge_synthetic",
+    "tm_tsm_batch_host_bits", "tm_noise_z4", "tm_gauge_fix_temporal", "tm_kernel_signature", "tm_gauge_synthetic", "tm_loop_contract_static",
 ]
 
 
@@ -101,6 +103,7 @@ def load():
         "tm_kernel_timing_enable": (i, [i]),
         "tm_kernel_timing_read": (i, [P(d), P(ctypes.c_longlong), i]),
         "tm_kernel_signature": (ctypes.c_char_p, []),
+        "tm_loop_contract_static": (i, [vp, vp, vp, i, i, vp, vp]),
         "tm_gauge_synthetic": (i, [vp, ctypes.c_ulonglong, d, d, vp, vp]),
         "tm_covdev": (i, [vp, vp, i, i, vp, vp, i, i, vp]),
         "tm_contract_field": (i, [vp, vp, vp, i, i, vp, vp]),
@@ -385,6 +388,11 @@ def tm_kernel_timing_read(reset=True):
     n = ctypes.c_longlong()
     _check(load().tm_kernel_timing_read(ctypes.byref(ms), ctypes.byref(n), int(reset)), "tm_kernel_timing_read")
     return ms.value, n.value
+
+
+def tm_loop_contract_static(L, a_full, b_full, prec, nrhs, out, stream=None):
+    return _check(load().tm_loop_contract_static(L.handle, _ptr(a_full), _ptr(b_full), prec, nrhs, _ptr(out), _stream(stream)),
+                  "tm_loop_contract_static")
 
 
 def tm_kernel_signature():

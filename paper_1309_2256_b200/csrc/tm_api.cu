@@ -110,6 +110,7 @@ extern "C" const char* tm_strerror(int s)
     case TM_ERR_CUDA: return "CUDA runtime error (see tm_last_cuda_error)";
     case TM_ERR_BREAKDOWN: return "CG breakdown (<p,Ap> <= 0 or NaN)";
     case TM_ERR_MAXITER: return "CG reached max_iter before the requested tolerance";
+    case TM_ERR_STATIC_LIMIT: return "tm_loop_contract_static: nrhs * T * blocks needs more than the TM_LOOP_STATIC_BYTES (8 MiB) static scratch array; use tm_loop_contract with a workspace";
     default: return "unknown status";
     }
 }

@@ -12,6 +12,7 @@
 #include "tm_layout.cuh"
 #include "tm_gamma.cuh"
 #include "tm_contract.cuh"
+#include <mutex>
 
 namespace tmk {
 
@@ -199,6 +200,44 @@ extern "C" int tm_loop_contract_ex(const tm_lattice* L, const void* a_full, cons
     if (!aligned256(a_full) || !aligned256(b_full) || !aligned256(out) || !aligned256(workspace)) return TM_ERR_LAYOUT;
     return loop_contract_ex(L->g, a_full, b_full, prec, nrhs, out, workspace, g5_left != 0, g5_right != 0, scale_re, scale_im,
                             (cudaStream_t)stream);
+}
+
+/* ---- the loop contraction for callers that cannot allocate (tm.h: tm_loop_contract_static) --------------------------------
+ * Same two kernels as tm_loop_contract; the per-block partial sums go to a file-scope device array instead of a caller workspace.
+ * In host code `g_loop_scratch` is only the host-side stand-in of the symbol, NOT a device address: the address is looked up once
+ * per device (with that device current) by cudaGetSymbolAddress and that pointer is what the kernels get. */
+static __device__ __align__(256) unsigned char g_loop_scratch[TM_LOOP_STATIC_BYTES];
+
+static int loop_scratch_ptr(void** out)
+{
+    constexpr int MAX_DEV = 64;
+    static std::mutex mu;
+    static void* ptrs[MAX_DEV] = {};
+    int dev = -1;
+    TM_CUDA_CHECK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEV) return TM_ERR_ARG;
+    std::lock_guard<std::mutex> lk(mu);
+    if (ptrs[dev] == nullptr) {
+        void* p = nullptr;
+        TM_CUDA_CHECK(cudaGetSymbolAddress(&p, g_loop_scratch));
+        if (p == nullptr) return TM_ERR_CUDA;
+        ptrs[dev] = p;
+    }
+    *out = ptrs[dev];
+    return TM_OK;
+}
+
+extern "C" int tm_loop_contract_static(const tm_lattice* L, const void* a_full, const void* b_full, int prec, int nrhs, double* out,
+                                       void* stream)
+{
+    if (!L || !a_full || !b_full || !out || !valid_prec(prec) || nrhs < 1) return TM_ERR_ARG;
+    if (!aligned256(a_full) || !aligned256(b_full) || !aligned256(out)) return TM_ERR_LAYOUT;
+    if (loop_workspace_bytes(L->g, nrhs) > (size_t)TM_LOOP_STATIC_BYTES) return TM_ERR_STATIC_LIMIT;
+    void* scratch = nullptr;
+    const int rc = loop_scratch_ptr(&scratch);
+    if (rc != TM_OK) return rc;
+    // nothing has to start at zero: loop_partial_kernel writes every partial that loop_final_kernel reads
+    return loop_contract(L->g, a_full, b_full, prec, nrhs, out, scratch, (cudaStream_t)stream);
 }
 
 /* single-time-slice contraction, used with time-diluted sources */

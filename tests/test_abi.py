@@ -29,7 +29,7 @@ def test_every_declared_symbol_is_exported(tm):
 
 def test_version_and_errors(tm):
     assert tm.tm_version() == 100
-    for s in range(0, -9, -1):
+    for s in range(0, -10, -1):
         assert tm.tm_strerror(s) != "unknown status"
     assert tm.tm_strerror(-99) == "unknown status"
 
@@ -90,6 +90,7 @@ def test_every_wrapper_reaches_the_library(tm):
         lambda: tm.tm_cg_multi(L, None, 8, None, 4, 18, buf, buf, prm, 2, buf, stream=0),
         lambda: tm.tm_cg(L, None, 8, None, 4, 18, buf, buf, prm, buf, stream=0),
         lambda: tm.tm_loop_contract(L, None, buf, 4, 1, buf, buf, stream=0),
+        lambda: tm.tm_loop_contract_static(L, None, buf, 4, 1, buf, stream=0),
         lambda: tm.tm_loop_contract_ex(L, None, buf, 4, 1, 1, 0, 2j, buf, buf, stream=0),
         lambda: tm.tm_loop_contract_slice(L, None, buf, 4, 1, 0, buf, buf, stream=0),
         lambda: tm.tm_loop_momentum(L, None, buf, 4, 1, mom, buf, buf, stream=0),
