@@ -680,7 +680,11 @@ __global__ void __launch_bounds__(32 * RB, MINB) dslash_tile_lc_kernel(const Dsl
     const int rhs = by * RB + ty;
     const bool ract = rhs < a.nrhs && (a.active == nullptr || a.active[rhs] != 0);
     const bool leader = (tx == 0 && ty == 0);
+#ifdef TM_DEBUG_IMGWIN // timing ablation (probe builds only, wrong results): all tile images from a 64-tile window (L2 hits, no DRAM traffic)
+    const char* img = a.link_cache + ((size_t)a.parity * tiles + (tile0 & 63)) * sizeof(TileSmem<S>);
+#else
     const char* img = a.link_cache + ((size_t)a.parity * tiles + tile0) * sizeof(TileSmem<S>);
+#endif
     if (leader) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&bar[0])) : "memory");
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&bar[1])) : "memory");
