@@ -573,7 +573,7 @@ int cg_hp_defect(const Geo& g, const void* gauge_hp, int prec_hp, const void* ga
     r2 = b2;
     tm_cg_params inner = *prm;
     inner.mode = TM_CG_LP_TRUNCATED;
-    inner.tol = (prm->reliable_delta > 0 && prm->reliable_delta < 1) ? prm->reliable_delta : 3e-3;
+    inner.tol = (prm->reliable_delta > 0 && prm->reliable_delta < 1) ? prm->reliable_delta : 1e-3;
     inner.skip_true_resid = 1;
     inner.check_every = 0;
     std::vector<tm_cg_info> iinfo(nrhs);
@@ -601,7 +601,7 @@ int cg_hp_defect(const Geo& g, const void* gauge_hp, int prec_hp, const void* ga
         double worst_rel = 0.0;
         for (int q = 0; q < nrhs; ++q)
             if (b2[q] > 0) worst_rel = std::max(worst_rel, std::sqrt(r2[q] / b2[q]));
-        const double base_tol = (prm->reliable_delta > 0 && prm->reliable_delta < 1) ? prm->reliable_delta : 3e-3;
+        const double base_tol = (prm->reliable_delta > 0 && prm->reliable_delta < 1) ? prm->reliable_delta : 1e-3;
         inner.tol = worst_rel > 0 ? std::min(0.5, std::max(base_tol, 0.3 * prm->tol / worst_rel)) : base_tol;
         if ((rc = k_convert(g, prec_lp, prec_hp, V_(r_lp, pbl), VecArg{nullptr, 0}, V_(R, pbh), nv, st)) != TM_OK) return rc;
         rc = cg_lp_truncated(g, gauge_lp, prec_lp, recon, e_lp, r_lp, &inner, nrhs, iinfo.data(), lpws, lpb, st);
