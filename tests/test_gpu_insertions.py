@@ -73,7 +73,10 @@ def test_contract_field(prec):
 
 
 @pytest.mark.parametrize("prec", [8, 4, 2])
-@pytest.mark.parametrize("dims,p2max", [((4, 6, 8, 10), 9), ((8, 8, 8, 4), 14), ((16, 16, 16, 4), 9)])
+@pytest.mark.parametrize("dims,p2max", [((4, 6, 8, 10), 9), ((8, 8, 8, 4), 14), ((16, 16, 16, 4), 9),
+                                        # the row kernel's other shapes: two sites per lane (X = 64), X / 2 odd and more than four
+                                        # row-warps per plane (Y = 40), the unrolled X = 32 form with a single warp and a ragged row count
+                                        ((64, 4, 4, 4), 9), ((12, 40, 4, 4), 9), ((32, 6, 4, 4), 5)])
 def test_loop_momentum(prec, dims, p2max):
     """Fused contraction + partial DFT against the plain nested sums; the p^2 <= 9 list of PAPER.md:427 (123 momenta), and a
     larger list reaching |m_i| = 3 with several y-row passes and a ragged last pass (Y = 6)."""
