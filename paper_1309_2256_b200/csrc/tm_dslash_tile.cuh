@@ -680,24 +680,35 @@ __global__ void __launch_bounds__(32 * RB, MINB) dslash_tile_lc_kernel(const Dsl
     const int rhs = by * RB + ty;
     const bool ract = rhs < a.nrhs && (a.active == nullptr || a.active[rhs] != 0);
     const bool leader = (tx == 0 && ty == 0);
-#ifdef TM_DEBUG_IMGWIN // timing ablation (probe builds only, wrong results): all tile images from a 64-tile window (L2 hits, no DRAM traffic)
-    const char* img = a.link_cache + ((size_t)a.parity * tiles + (tile0 & 63)) * sizeof(TileSmem<S>);
-#else
     const char* img = a.link_cache + ((size_t)a.parity * tiles + tile0) * sizeof(TileSmem<S>);
+#ifdef TM_DEBUG_IMGWIN
+    // timing ablation (probe builds only, wrong results): the LINKS of every tile image come from a 64-tile window of the cache (L2
+    // hits, no DRAM traffic), the neighbour indices from the tile's own image (the gathers keep their addresses): two copies per image
+    constexpr uint32_t NBYTES = (uint32_t)sizeof(((TileSmem<S>*)nullptr)->nbr);
+    const char* imgw = a.link_cache + ((size_t)a.parity * tiles + (tile0 & 63)) * sizeof(TileSmem<S>);
+#define TM_IMG_LOAD(buf, k)                                                                                              \
+    do {                                                                                                                 \
+        bulk_load(smem_u32(&sm[buf]), img + (size_t)(k) * sizeof(TileSmem<S>), NBYTES, smem_u32(&bar[buf]));             \
+        bulk_load(smem_u32(&sm[buf]) + NBYTES, imgw + (size_t)((k) & 3) * sizeof(TileSmem<S>) + NBYTES, BYTES - NBYTES, smem_u32(&bar[buf])); \
+    } while (0)
+    constexpr int ARRIVALS = 2;
+#else
+#define TM_IMG_LOAD(buf, k) bulk_load(smem_u32(&sm[buf]), img + (size_t)(k) * sizeof(TileSmem<S>), BYTES, smem_u32(&bar[buf]))
+    constexpr int ARRIVALS = 1;
 #endif
     if (leader) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&bar[0])) : "memory");
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(&bar[1])) : "memory");
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(&bar[0])), "r"(ARRIVALS) : "memory");
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(&bar[1])), "r"(ARRIVALS) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (__syncthreads_or(ract) == 0) return;
-    if (leader) bulk_load(smem_u32(&sm[0]), img, BYTES, smem_u32(&bar[0]));
+    if (leader) TM_IMG_LOAD(0, 0);
     // (decoupling the warps with per-buffer "empty" mbarriers instead of the CTA barrier was measured 2 % slower; two to six
     // right-hand sides per thread with the links kept in registers 15 % to 4.8 x slower: profiles/r02_ablations_12rhs_dslash.md)
     for (int i = 0; i < ntile; ++i) {
         const int b = i & 1;
         if (leader && i + 1 < ntile) // buffer b^1 was released by the barrier that closed tile i-1
-            bulk_load(smem_u32(&sm[b ^ 1]), img + (size_t)(i + 1) * sizeof(TileSmem<S>), BYTES, smem_u32(&bar[b ^ 1]));
+            TM_IMG_LOAD(b ^ 1, i + 1);
         const int cb = (tile0 + i) * S + tx;
         if (ract && cb < Vh) {
             mbar_wait(smem_u32(&bar[b]), (i >> 1) & 1);
@@ -712,6 +723,8 @@ __global__ void __launch_bounds__(32 * RB, MINB) dslash_tile_lc_kernel(const Dsl
         if (i + 1 < ntile) __syncthreads();
     }
 }
+
+#undef TM_IMG_LOAD
 
 template <int PREC, int RECON, int RB, int MINB, int TPC>
 static inline void launch_tile_lc(const DslashKArgs& a, bool dagger, cudaStream_t st)
