@@ -304,9 +304,10 @@ __global__ void __launch_bounds__(FIN_THREADS) dot_finalize_kernel(const double*
 }
 
 // iteration `iter` (0-based): x += alpha p for every rhs whose alpha belongs to this iteration (also the one that has just
-// converged); p = r + beta p for the rhs that are still active
+// converged); p = r + beta p for the rhs that are still active.  The search direction is read from pin_ and written to p_ (the
+// same stack from iteration 1 on; in iteration 0 pin_ is the right-hand side b itself, p_0 = r_0 = b, so no copies of b are made)
 template <int PREC>
-__global__ void __launch_bounds__(BLAS_THREADS) update_xp_kernel(int Vh, VecArg x_, VecArg p_, VecArg r_, BlasCtx c, int iter)
+__global__ void __launch_bounds__(BLAS_THREADS) update_xp_kernel(int Vh, VecArg x_, VecArg p_, VecArg pin_, VecArg r_, BlasCtx c, int iter)
 {
     typedef typename Prec<PREC>::real real;
     const int rhs = blockIdx.y;
@@ -316,7 +317,7 @@ __global__ void __launch_bounds__(BLAS_THREADS) update_xp_kernel(int Vh, VecArg 
     for (int cb = blockIdx.x * BLAS_THREADS + threadIdx.x; cb < Vh; cb += gridDim.x * BLAS_THREADS) {
         real x[24], p[24];
         load_spinor<PREC>(x_.p + rhs * x_.stride, Vh, cb, x);
-        load_spinor<PREC>(p_.p + rhs * p_.stride, Vh, cb, p);
+        load_spinor<PREC>(pin_.p + rhs * pin_.stride, Vh, cb, p);
 #pragma unroll
         for (int k = 0; k < 24; ++k) x[k] = fma(alpha, p[k], x[k]);
         store_spinor<PREC>(x_.p + rhs * x_.stride, Vh, cb, x);

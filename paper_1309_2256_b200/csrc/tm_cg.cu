@@ -96,8 +96,11 @@ static int k_cg_iter(const Geo& g, const void* gauge, int prec, int recon, VecAr
 //   t1 = R(-a)^-1 D^dag t2;  r = r - alpha (R(-a) t2 - kappa^2 D^dag t1), partials of |r|^2;  [finalize -> beta, convergence]
 //   x += alpha p, p = r + beta p.
 // A p is never written to memory; the only vector kernel left moves 5 one-parity spinors per rhs (11 before).
-static int k_cg_iter_fused(const Geo& g, const void* gauge, int prec, int recon, VecArg x, VecArg r, VecArg p, void* tmp, double kappa,
-                           double mu, const BlasCtx& c, double* partial, int nrhs, int iter, cudaStream_t st, const void* link_cache)
+// pin / rin: where this iteration READS its search direction and residual (the stacks p / r themselves from iteration 1 on; the
+// right-hand side b in iteration 0, where p_0 = r_0 = b: the solver makes no copies of b).
+static int k_cg_iter_fused(const Geo& g, const void* gauge, int prec, int recon, VecArg x, VecArg r, VecArg p, VecArg rin, VecArg pin,
+                           void* tmp, double kappa, double mu, const BlasCtx& c, double* partial, int nrhs, int iter, cudaStream_t st,
+                           const void* link_cache)
 {
     const size_t pb = spinor_parity_bytes(g, prec);
     char* t1 = static_cast<char*>(tmp);
@@ -107,10 +110,10 @@ static int k_cg_iter_fused(const Geo& g, const void* gauge, int prec, int recon,
     d.gauge = gauge; d.nrhs = nrhs; d.active = c.active; d.link_cache = link_cache;
     d.rhs_stride_out = d.rhs_stride_in = d.rhs_stride_x = pb;
     int rc;
-    d.out = t1; d.in = p.p; d.x = nullptr; d.out_parity = 1; d.dagger = 0; d.rhs_stride_in = p.stride;
+    d.out = t1; d.in = pin.p; d.x = nullptr; d.out_parity = 1; d.dagger = 0; d.rhs_stride_in = pin.stride;
     kind_pq(TM_KIND_TWIST_INV, 0, kappa, mu, d.pq);
     if ((rc = launch_dslash(g, prec, recon, d, st)) != TM_OK) return rc;
-    d.out = t2; d.in = t1; d.x = p.p; d.out_parity = 0; d.rhs_stride_in = pb; d.rhs_stride_x = p.stride;
+    d.out = t2; d.in = t1; d.x = pin.p; d.out_parity = 0; d.rhs_stride_in = pb; d.rhs_stride_x = pin.stride;
     kind_pq(TM_KIND_XPAY_TWIST, 0, kappa, mu, d.pq);
     d.dot_partial = partial;
     if ((rc = launch_dslash(g, prec, recon, d, st)) != TM_OK) return rc;
@@ -122,7 +125,7 @@ static int k_cg_iter_fused(const Geo& g, const void* gauge, int prec, int recon,
     if ((rc = launch_dslash(g, prec, recon, d, st)) != TM_OK) return rc;
     d.out = r.p; d.in = t1; d.x = t2; d.out_parity = 0; d.rhs_stride_out = r.stride;
     kind_pq(TM_KIND_XPAY_TWIST, 1, kappa, mu, d.pq);
-    d.axpy_y = r.p; d.axpy_y_stride = r.stride;
+    d.axpy_y = rin.p; d.axpy_y_stride = rin.stride;
     d.axpy_coef = &c.scal[0].alpha; d.axpy_coef_stride = sizeof(CgScal);
     d.dot_partial = partial;
     if ((rc = launch_dslash(g, prec, recon, d, st)) != TM_OK) return rc;
@@ -130,7 +133,7 @@ static int k_cg_iter_fused(const Geo& g, const void* gauge, int prec, int recon,
     TM_LAUNCH_CHECK("dot_finalize_kernel");
     dim3 grid(blas_blocks(g.Vh), nrhs);
     return by_prec(prec, [&](auto P) {
-        update_xp_kernel<decltype(P)::value><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, x, p, r, c, iter);
+        update_xp_kernel<decltype(P)::value><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, x, p, pin, r, c, iter);
         TM_LAUNCH_CHECK("update_xp_kernel");
         return (int)TM_OK;
     });
@@ -330,7 +333,7 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
     if (lc && (rc = link_cache_build(g, prec, recon, gauge, lc, st)) != TM_OK) return rc;
     if ((rc = prepare_rhs(g, gauge, prec, recon, eta_full, b, t1, t2, prm->kappa, prm->mu, nrhs, st, lc)) != TM_OK) return rc;
     if ((rc = k_norm2<FIN_INIT>(g, prec, V_(b, pb), c, nrhs, st)) != TM_OK) return rc;
-    if ((rc = k_convert(g, prec, prec, V_(r, pb), V_(p, pb), V_(b, pb), nrhs, st)) != TM_OK) return rc;
+    // r_0 = p_0 = b: iteration 0 reads both from b (k_cg_iter_fused), the stacks r and p are first written by it
     VecArg x = V_(s_full, 2 * pb); // s_e lives in the even block of s_full
     TM_CUDA_CHECK(cudaMemset2DAsync(s_full, 2 * pb, 0, pb, nrhs, st));
     if (prm->check_every > 0) {
@@ -339,8 +342,8 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
         unsigned char hact[TM_MAX_NRHS];
         for (int k = 0; k < prm->max_iter;) {
             for (int j = 0; j < every && k < prm->max_iter; ++j, ++k)
-                if ((rc = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), t1, prm->kappa, prm->mu, c, dotp, nrhs, k,
-                                          st, lc)) != TM_OK)
+                if ((rc = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), V_(k == 0 ? b : r, pb), V_(k == 0 ? b : p, pb), t1,
+                                          prm->kappa, prm->mu, c, dotp, nrhs, k, st, lc)) != TM_OK)
                     return rc;
             TM_CUDA_CHECK(cudaMemcpyAsync(hact, c.active, nrhs, cudaMemcpyDeviceToHost, st));
             TM_CUDA_CHECK(cudaStreamSynchronize(st));
@@ -355,8 +358,8 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
         PollRing* ring = poll_ring();
         if (!ring) return TM_ERR_CUDA;
         for (int k = 0; k < prm->max_iter; ++k) {
-            if ((rc = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), t1, prm->kappa, prm->mu, c, dotp, nrhs, k, st,
-                                      lc)) != TM_OK)
+            if ((rc = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), V_(k == 0 ? b : r, pb), V_(k == 0 ? b : p, pb), t1,
+                                      prm->kappa, prm->mu, c, dotp, nrhs, k, st, lc)) != TM_OK)
                 return rc;
             const int slot = k % PollRing::DEPTH;
             TM_CUDA_CHECK(cudaMemcpyAsync(ring->flags + slot * TM_MAX_NRHS, c.active, nrhs, cudaMemcpyDeviceToHost, st));
