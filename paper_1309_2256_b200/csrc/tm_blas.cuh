@@ -311,12 +311,28 @@ __global__ void __launch_bounds__(BLAS_THREADS) update_xp_kernel(int Vh, VecArg 
 {
     typedef typename Prec<PREC>::real real;
     const int rhs = blockIdx.y;
-    if (c.scal[rhs].alpha_iter != iter || c.scal[rhs].alpha == 0.0) return;
+    if (c.scal[rhs].alpha_iter != iter || c.scal[rhs].alpha == 0.0) {
+        // iteration 0 also sets the initial guess x_0 = 0 (no memset, no read of x): a right-hand side that does not iterate (zero
+        // source, breakdown in the first step) gets its zeros here
+        if (iter == 0) {
+            real z[24];
+#pragma unroll
+            for (int k = 0; k < 24; ++k) z[k] = 0;
+            for (int cb = blockIdx.x * BLAS_THREADS + threadIdx.x; cb < Vh; cb += gridDim.x * BLAS_THREADS)
+                store_spinor<PREC>(x_.p + rhs * x_.stride, Vh, cb, z);
+        }
+        return;
+    }
     const bool more = c.active[rhs] != 0;
     const real alpha = (real)c.scal[rhs].alpha, beta = (real)c.scal[rhs].beta;
     for (int cb = blockIdx.x * BLAS_THREADS + threadIdx.x; cb < Vh; cb += gridDim.x * BLAS_THREADS) {
         real x[24], p[24];
-        load_spinor<PREC>(x_.p + rhs * x_.stride, Vh, cb, x);
+        if (iter == 0) {
+#pragma unroll
+            for (int k = 0; k < 24; ++k) x[k] = 0;
+        } else {
+            load_spinor<PREC>(x_.p + rhs * x_.stride, Vh, cb, x);
+        }
         load_spinor<PREC>(pin_.p + rhs * pin_.stride, Vh, cb, p);
 #pragma unroll
         for (int k = 0; k < 24; ++k) x[k] = fma(alpha, p[k], x[k]);

@@ -335,7 +335,8 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
     if ((rc = k_norm2<FIN_INIT>(g, prec, V_(b, pb), c, nrhs, st)) != TM_OK) return rc;
     // r_0 = p_0 = b: iteration 0 reads both from b (k_cg_iter_fused), the stacks r and p are first written by it
     VecArg x = V_(s_full, 2 * pb); // s_e lives in the even block of s_full
-    TM_CUDA_CHECK(cudaMemset2DAsync(s_full, 2 * pb, 0, pb, nrhs, st));
+    // x_0 = 0 is written by the vector kernel of iteration 0; only a solve without any iteration needs the memset
+    if (prm->max_iter < 1) TM_CUDA_CHECK(cudaMemset2DAsync(s_full, 2 * pb, 0, pb, nrhs, st));
     if (prm->check_every > 0) {
         // poll the device flags every `check_every` iterations (one stream synchronisation per poll)
         const int every = prm->check_every;

@@ -101,6 +101,21 @@ def test_cg_zero_source_and_mixed_convergence_times():
     assert rc == tm.TM_OK and info[1].iters == 0 and not s[1].any()
     for r in (0, 2):
         assert rel(oracle.M(U, s[r], KAPPA, MU), eta[r]) < 1e-4
+    # x_0 = 0 is the solver's own business (written by the first iteration's vector kernel, or by a memset when max_iter = 0): a
+    # solution buffer full of garbage changes nothing, and the zero source still gets an all-zero solution
+    for prec, max_iter in ((4, 500), (2, 500), (4, 0)):
+        pe = F.pack(eta, prec)
+        sd = tm.device_buffer(tm.tm_spinor_bytes(F.L, prec, 1, 3))
+        sd.fill_(0x3C)
+        ws = tm.device_buffer(tm.tm_cg_workspace_bytes(F.L, 8, prec, tm.TM_CG_LP_TRUNCATED, 3))
+        prm = tm.make_cg_params(KAPPA, MU, 1e-2, max_iter, tm.TM_CG_LP_TRUNCATED)
+        rc2, info2 = tm.tm_cg_multi(F.L, None, 8, F.gauge(prec, 18), prec, 18, sd, pe, prm, 3, ws)
+        got = F.unpack(sd, prec, nrhs=3)
+        assert not got[1].any() and np.isfinite(got).all()
+        if max_iter == 0:
+            assert not oracle.project(got[0], 0).any()   # no iteration: s_e = x_0 = 0, s_o = R^-1 eta_o
+        else:
+            assert rc2 == tm.TM_OK and rel(oracle.M(U, got[0], KAPPA, MU), eta[0]) < 3e-2
 
 
 def test_skip_true_resid_changes_nothing_but_the_report():
