@@ -347,6 +347,78 @@ __global__ void __launch_bounds__(BLAS_THREADS) update_xp_kernel(int Vh, VecArg 
     }
 }
 
+// ---- search-direction ring of the truncated solver ------------------------------------------------------------------
+// With room for LP_RING_DEPTH search directions the solution is not touched inside the iteration: iteration k only forms
+// p_{k+1} = r_{k+1} + beta_k p_k into the next ring slot (three vector passes instead of five) and records alpha_k;
+// x += sum_k alpha_k p_k is formed every LP_FLUSH_EVERY iterations and at the end in one pass over the kept directions (fp32 / fp64
+// registers, one rounding to storage per pass).  Depth and schedule are constants, so a right-hand side gets the same bits whether
+// it is solved alone or in a batch.
+constexpr int LP_RING_DEPTH = 10;
+constexpr int LP_FLUSH_EVERY = 8;
+
+// p_out = r + beta p_in for the right-hand sides still active; hist[rhs] = alpha of iteration `iter` (0 if the rhs did not iterate)
+template <int PREC>
+__global__ void __launch_bounds__(BLAS_THREADS) update_p_hist_kernel(int Vh, VecArg pout_, VecArg pin_, VecArg r_, BlasCtx c, int iter,
+                                                                     double* hist)
+{
+    typedef typename Prec<PREC>::real real;
+    const int rhs = blockIdx.y;
+    const double a = (c.scal[rhs].alpha_iter == iter) ? c.scal[rhs].alpha : 0.0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) hist[rhs] = a;
+    if (a == 0.0 || c.active[rhs] == 0) return;
+    const real beta = (real)c.scal[rhs].beta;
+    for (int cb = blockIdx.x * BLAS_THREADS + threadIdx.x; cb < Vh; cb += gridDim.x * BLAS_THREADS) {
+        real p[24], r[24];
+        load_spinor<PREC>(pin_.p + rhs * pin_.stride, Vh, cb, p);
+        load_spinor<PREC>(r_.p + rhs * r_.stride, Vh, cb, r);
+#pragma unroll
+        for (int k = 0; k < 24; ++k) p[k] = fma(beta, p[k], r[k]);
+        store_spinor<PREC>(pout_.p + rhs * pout_.stride, Vh, cb, p);
+    }
+}
+
+struct XTerms {
+    const char* p[LP_FLUSH_EVERY];      // search directions (stacks over the right-hand sides)
+    size_t stride[LP_FLUSH_EVERY];
+    const double* alpha[LP_FLUSH_EVERY]; // their coefficients, [rhs]
+    int n;
+};
+
+// x = (init ? 0 : x) + sum_{j < n} alpha_j p_j, terms in the order given, per right-hand side
+template <int PREC>
+__global__ void __launch_bounds__(BLAS_THREADS) accumulate_x_kernel(int Vh, VecArg x_, XTerms t, int init)
+{
+    typedef typename Prec<PREC>::real real;
+    const int rhs = blockIdx.y;
+    real a[LP_FLUSH_EVERY];
+    bool any = false;
+#pragma unroll
+    for (int j = 0; j < LP_FLUSH_EVERY; ++j) {
+        a[j] = j < t.n ? (real)t.alpha[j][rhs] : real(0);
+        any |= a[j] != real(0);
+    }
+    if (!any && !init) return;
+    for (int cb = blockIdx.x * BLAS_THREADS + threadIdx.x; cb < Vh; cb += gridDim.x * BLAS_THREADS) {
+        real x[24];
+        if (init) {
+#pragma unroll
+            for (int k = 0; k < 24; ++k) x[k] = 0;
+        } else {
+            load_spinor<PREC>(x_.p + rhs * x_.stride, Vh, cb, x);
+        }
+#pragma unroll
+        for (int j = 0; j < LP_FLUSH_EVERY; ++j) {
+            if (j < t.n && a[j] != real(0)) {
+                real p[24];
+                load_spinor<PREC>(t.p[j] + rhs * t.stride[j], Vh, cb, p);
+#pragma unroll
+                for (int k = 0; k < 24; ++k) x[k] = fma(a[j], p[k], x[k]);
+            }
+        }
+        store_spinor<PREC>(x_.p + rhs * x_.stride, Vh, cb, x);
+    }
+}
+
 static inline int blas_blocks(int Vh)
 {
     int nb = (Vh + BLAS_THREADS - 1) / BLAS_THREADS;

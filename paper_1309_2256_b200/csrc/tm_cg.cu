@@ -100,7 +100,7 @@ static int k_cg_iter(const Geo& g, const void* gauge, int prec, int recon, VecAr
 // right-hand side b in iteration 0, where p_0 = r_0 = b: the solver makes no copies of b).
 static int k_cg_iter_fused(const Geo& g, const void* gauge, int prec, int recon, VecArg x, VecArg r, VecArg p, VecArg rin, VecArg pin,
                            void* tmp, double kappa, double mu, const BlasCtx& c, double* partial, int nrhs, int iter, cudaStream_t st,
-                           const void* link_cache)
+                           const void* link_cache, bool do_xp = true)
 {
     const size_t pb = spinor_parity_bytes(g, prec);
     char* t1 = static_cast<char*>(tmp);
@@ -131,6 +131,7 @@ static int k_cg_iter_fused(const Geo& g, const void* gauge, int prec, int recon,
     if ((rc = launch_dslash(g, prec, recon, d, st)) != TM_OK) return rc;
     dot_finalize_kernel<FIN_RR><<<nrhs, FIN_THREADS, 0, st>>>(partial, ngroups, c);
     TM_LAUNCH_CHECK("dot_finalize_kernel");
+    if (!do_xp) return TM_OK; // the caller keeps the search directions in a ring and forms x afterwards
     dim3 grid(blas_blocks(g.Vh), nrhs);
     return by_prec(prec, [&](auto P) {
         update_xp_kernel<decltype(P)::value><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, x, p, pin, r, c, iter);
@@ -307,9 +308,23 @@ static int reconstruct_odd(const Geo& g, const void* gauge, int prec, int recon,
 static inline bool lp_uses_link_cache(int prec, int nrhs) { return prec != 8 && nrhs > 6; }
 static inline size_t dot_partial_bytes(const Geo& g, int nrhs) { return round256(sizeof(double) * (size_t)((g.Vh + 31) / 32) * nrhs); }
 
+// Search-direction ring (tm_blas.cuh): used when its LP_RING_DEPTH - 1 extra stacks fit into TM_LP_RING_BYTES; otherwise the solution
+// is updated inside the iteration (five vector passes per iteration instead of three + one pass per direction at a flush).
+#ifndef TM_LP_RING_BYTES
+#define TM_LP_RING_BYTES (size_t(16) << 30)
+#endif
+static inline int lp_ring_depth(const Geo& g, int prec, int nrhs)
+{
+    return (size_t)(LP_RING_DEPTH - 1) * round256(spinor_parity_bytes(g, prec) * nrhs) <= TM_LP_RING_BYTES ? LP_RING_DEPTH : 1;
+}
+static inline size_t lp_hist_bytes(int depth, int nrhs) { return round256(sizeof(double) * (size_t)(depth + 1) * nrhs); }
+
 size_t cg_lp_workspace_bytes(const Geo& g, int prec, int nrhs)
 {
-    return ctx_bytes(nrhs) + dot_partial_bytes(g, nrhs) + 6 * round256(spinor_parity_bytes(g, prec) * nrhs) + (lp_uses_link_cache(prec, nrhs) ? link_cache_bytes(g, prec) : 0);
+    const int D = lp_ring_depth(g, prec, nrhs);
+    const size_t stack = round256(spinor_parity_bytes(g, prec) * nrhs);
+    return ctx_bytes(nrhs) + dot_partial_bytes(g, nrhs) + 6 * stack + (lp_uses_link_cache(prec, nrhs) ? link_cache_bytes(g, prec) : 0) +
+           (D >= 2 ? (size_t)(D - 1) * stack + lp_hist_bytes(D, nrhs) : 0);
 }
 
 // truncated LP solve, batched
@@ -327,6 +342,13 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
     void* t2 = static_cast<char*>(t1) + pb * nrhs;
     void* lc = lp_uses_link_cache(prec, nrhs) ? cv.take(link_cache_bytes(g, prec)) : nullptr;
     double* dotp = static_cast<double*>(cv.take(dot_partial_bytes(g, nrhs)));
+    const int D = lp_ring_depth(g, prec, nrhs);
+    void* ringbuf[LP_RING_DEPTH] = {p};
+    double* hist = nullptr;
+    if (D >= 2) {
+        for (int j = 1; j < D; ++j) ringbuf[j] = cv.take(pb * nrhs);
+        hist = static_cast<double*>(cv.take(sizeof(double) * (size_t)(D + 1) * nrhs));
+    }
     if (!cv.ok()) return TM_ERR_LAYOUT;
     int rc;
     if ((rc = init_ctx(c, prm, nrhs, st)) != TM_OK) return rc;
@@ -335,17 +357,64 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
     if ((rc = k_norm2<FIN_INIT>(g, prec, V_(b, pb), c, nrhs, st)) != TM_OK) return rc;
     // r_0 = p_0 = b: iteration 0 reads both from b (k_cg_iter_fused), the stacks r and p are first written by it
     VecArg x = V_(s_full, 2 * pb); // s_e lives in the even block of s_full
-    // x_0 = 0 is written by the vector kernel of iteration 0; only a solve without any iteration needs the memset
-    if (prm->max_iter < 1) TM_CUDA_CHECK(cudaMemset2DAsync(s_full, 2 * pb, 0, pb, nrhs, st));
+    // x_0 = 0 is written by the vector kernel of iteration 0 (or by the first accumulation of the ring); only a solve without any
+    // iteration and without a ring needs the memset
+    if (prm->max_iter < 1 && D < 2) TM_CUDA_CHECK(cudaMemset2DAsync(s_full, 2 * pb, 0, pb, nrhs, st));
+    // search direction p_j lives in b (j = 0) or in ring slot (j - 1) % D
+    auto slot = [&](int j) -> void* { return j == 0 ? b : ringbuf[(j - 1) % D]; };
+    int flushed = 0;      // x holds sum_{j < flushed} alpha_j p_j
+    bool x_init = true;   // the first accumulation writes x instead of adding to it
+    auto flush = [&](int upto) -> int {
+        if (upto <= flushed && !x_init) return (int)TM_OK;
+        XTerms t;
+        t.n = 0;
+        for (int j = flushed; j < upto; ++j, ++t.n) {
+            t.p[t.n] = static_cast<const char*>(slot(j));
+            t.stride[t.n] = pb;
+            t.alpha[t.n] = hist + (size_t)(j % (D + 1)) * nrhs;
+        }
+        dim3 grid(blas_blocks(g.Vh), nrhs);
+        const int init = x_init ? 1 : 0;
+        const int rcf = by_prec(prec, [&](auto P) {
+            accumulate_x_kernel<decltype(P)::value><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, x, t, init);
+            TM_LAUNCH_CHECK("accumulate_x_kernel");
+            return (int)TM_OK;
+        });
+        flushed = upto > flushed ? upto : flushed;
+        x_init = false;
+        return rcf;
+    };
+    // one iteration: the fused operator launches, then either the classic x / p update or the ring update
+    auto iterate = [&](int k) -> int {
+        if (D < 2)
+            return k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), V_(k == 0 ? b : r, pb), V_(k == 0 ? b : p, pb), t1, prm->kappa,
+                                   prm->mu, c, dotp, nrhs, k, st, lc);
+        void* pin = slot(k);
+        void* pout = ringbuf[k % D];
+        int rci = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(pout, pb), V_(k == 0 ? b : r, pb), V_(pin, pb), t1, prm->kappa, prm->mu, c,
+                                  dotp, nrhs, k, st, lc, false);
+        if (rci != TM_OK) return rci;
+        // p_{k+1} overwrites p_{k+1-D}: flushing every LP_FLUSH_EVERY < D - 1 iterations keeps every unflushed direction alive
+        if (k - flushed >= LP_FLUSH_EVERY && (rci = flush(k)) != TM_OK) return rci;
+        dim3 grid(blas_blocks(g.Vh), nrhs);
+        return by_prec(prec, [&](auto P) {
+            update_p_hist_kernel<decltype(P)::value><<<grid, BLAS_THREADS, 0, st>>>(g.Vh, V_(pout, pb), V_(pin, pb), V_(r, pb), c, k,
+                                                                                  hist + (size_t)(k % (D + 1)) * nrhs);
+            TM_LAUNCH_CHECK("update_p_hist_kernel");
+            return (int)TM_OK;
+        });
+    };
+    int launched = 0; // iterations launched
     if (prm->check_every > 0) {
         // poll the device flags every `check_every` iterations (one stream synchronisation per poll)
         const int every = prm->check_every;
         unsigned char hact[TM_MAX_NRHS];
         for (int k = 0; k < prm->max_iter;) {
             for (int j = 0; j < every && k < prm->max_iter; ++j, ++k)
-                if ((rc = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), V_(k == 0 ? b : r, pb), V_(k == 0 ? b : p, pb), t1,
-                                          prm->kappa, prm->mu, c, dotp, nrhs, k, st, lc)) != TM_OK)
-                    return rc;
+            {
+                if ((rc = iterate(k)) != TM_OK) return rc;
+                launched = k + 1;
+            }
             TM_CUDA_CHECK(cudaMemcpyAsync(hact, c.active, nrhs, cudaMemcpyDeviceToHost, st));
             TM_CUDA_CHECK(cudaStreamSynchronize(st));
             bool any = false;
@@ -359,9 +428,8 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
         PollRing* ring = poll_ring();
         if (!ring) return TM_ERR_CUDA;
         for (int k = 0; k < prm->max_iter; ++k) {
-            if ((rc = k_cg_iter_fused(g, gauge, prec, recon, x, V_(r, pb), V_(p, pb), V_(k == 0 ? b : r, pb), V_(k == 0 ? b : p, pb), t1,
-                                      prm->kappa, prm->mu, c, dotp, nrhs, k, st, lc)) != TM_OK)
-                return rc;
+            if ((rc = iterate(k)) != TM_OK) return rc;
+            launched = k + 1;
             const int slot = k % PollRing::DEPTH;
             TM_CUDA_CHECK(cudaMemcpyAsync(ring->flags + slot * TM_MAX_NRHS, c.active, nrhs, cudaMemcpyDeviceToHost, st));
             TM_CUDA_CHECK(cudaEventRecord(ring->ev[slot], st));
@@ -374,6 +442,7 @@ int cg_lp_truncated(const Geo& g, const void* gauge, int prec, int recon, void* 
             }
         }
     }
+    if (D >= 2 && (rc = flush(launched)) != TM_OK) return rc; // x = sum of the kept directions (zeros if nothing iterated)
     if ((rc = reconstruct_odd(g, gauge, prec, recon, s_full, eta_full, prm->kappa, prm->mu, nrhs, st, lc)) != TM_OK) return rc;
     // recomputed residual of the normal system, in the same storage/arithmetic: Ap = A x; Ap = b - Ap
     if (!prm->skip_true_resid) {
