@@ -353,8 +353,8 @@ __global__ void __launch_bounds__(BLAS_THREADS) update_xp_kernel(int Vh, VecArg 
 // x += sum_k alpha_k p_k is formed every LP_FLUSH_EVERY iterations and at the end in one pass over the kept directions (fp32 / fp64
 // registers, one rounding to storage per pass).  Depth and schedule are constants, so a right-hand side gets the same bits whether
 // it is solved alone or in a batch.
-constexpr int LP_RING_DEPTH = 10;
-constexpr int LP_FLUSH_EVERY = 8;
+constexpr int LP_RING_DEPTH = 14;
+constexpr int LP_FLUSH_EVERY = 12;
 
 // p_out = r + beta p_in for the right-hand sides still active; hist[rhs] = alpha of iteration `iter` (0 if the rhs did not iterate)
 template <int PREC>
