@@ -627,7 +627,7 @@ __global__ void __launch_bounds__(S* RB, MINB) dslash_tile_kernel(const DslashKA
 #pragma unroll
         for (int d = 0; d < 8; ++d) {
             const int v = sm.nbr[d][tx];
-            nb[d] = v < 0 ? ~v : v;
+            nb[d] = (d >= 6 && v < 0) ? ~v : v;
         }
     }
     float sgp = 1.f, sgm = 1.f;
@@ -716,7 +716,7 @@ __global__ void __launch_bounds__(32 * RB, MINB) dslash_tile_lc_kernel(const Dsl
 #pragma unroll
             for (int d = 0; d < 8; ++d) {
                 const int v = sm[b].nbr[d][tx];
-                nb[d] = v < 0 ? ~v : v;
+                nb[d] = (d >= 6 && v < 0) ? ~v : v; // only temporal hops carry the antiperiodic sign on their index
             }
             tile_site_any<PREC, RECON, DAG, 1>(a, sm[b], cb, tx, rhs, nb, 1.f, 1.f);
         }
