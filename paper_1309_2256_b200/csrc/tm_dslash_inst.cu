@@ -13,7 +13,7 @@
 #define TM_LC_MINB 2
 #endif
 #ifndef TM_LC_TPC
-#define TM_LC_TPC 4
+#define TM_LC_TPC 16
 #endif
 
 namespace tmk {
@@ -65,7 +65,8 @@ int launch_dslash_t<TM_PREC, TM_RECON>(const Geo& g, const DslashParams& p, cuda
     //   2..4 rhs   32 sites x 4 rhs, links of the tile built in shared memory, 6 CTAs/SM
     //   5..6 rhs   32 sites x 6 rhs, 4 CTAs/SM
     //   > 6 rhs    32 sites x 12 rhs, 2 CTAs/SM (80 registers); inside a solve the tile images come from the link cache
-    //              by cp.async.bulk, 4 tiles per CTA (7..8 rhs: 32 sites x 8 rhs, 3 CTAs/SM)
+    //              by cp.async.bulk, 16 tiles per CTA (7..8 rhs: 32 sites x 8 rhs, 3 CTAs/SM).  Tiles per CTA at 32^3x64: fp16
+    //              storage flat from 2 to 16 (332 solves/s), fp32 storage 237 / 242 / 248 solves/s at 4 / 8 / 16; 32 and more lose to the tail
     const bool dg = p.dagger != 0;
     if (n == 1) launch_tile<TM_PREC, TM_RECON, 128, 1, 4, 0>(a, dg, st);
     else if (n <= 4) launch_tile<TM_PREC, TM_RECON, 32, 4, 6, 1>(a, dg, st);
